@@ -1,0 +1,519 @@
+/* CPU ORACLE -- TEST INFRASTRUCTURE, NOT PRODUCT.  See ref_dg.h.
+ *
+ * Follows SURVEY.md section 8(c) step by step (readings G1..G20 are listed in DESIGN.md):
+ *   C1  tables          PAPER.md:65, 95-97, 155       Gauss-Legendre nodes/weights, phi_a = sqrt(2a+1) P_a
+ *   C2  nodal values    PAPER.md:73-75                u_h = sum_ab U_ab phi_a(xi) phi_b(eta)
+ *   C3  Euler fluxes    PAPER.md:36-43  Eq.(1)
+ *   C4  EOS             PAPER.md:45-49  Eq.(2); locally isothermal closure from BASELINE.json
+ *   C5  numerical flux  PAPER.md:97  (type unnamed; BASELINE cfg0: local Lax-Friedrichs)
+ *   C6  gravity source
+ *   C7  RHS             PAPER.md:85-97  Eq.(3), divided by the (diagonal) mass
+ *   C8  SSP-RK          PAPER.md:105-111 (Gottlieb & Shu 1998, Shu-Osher form)
+ *   C9  boundaries
+ *   C10 CFL
+ *   C11 wave damping
+ *
+ * No blocking, fusion, sum-factorisation or reordering: every sum is written as the nested loop
+ * the formula states, in fp64, compiled with -O2 -ffp-contract=off.
+ *
+ * Pins (tests/test_oracle_tables.py, test_oracle_pointwise.py, test_oracle_rhs.py,
+ * test_oracle_time.py; none of them re-types these formulas):
+ *   C1  sum w = 2; exactness on x^k, k <= 2m-1; closed forms m = 1,2,3; orthonormality; numpy leggauss
+ *   C3-C5  consistency H(U,U) = f(U).n; bitwise antisymmetry; Rankine-Hugoniot-free upwind limit
+ *   C6  centred finite difference of the potential; planet period 2 pi / Omega_p
+ *   C2+C7 volume term: 24-point brute-force quadrature of int_K f(u_h).grad(phi) (exact integrands)
+ *   C7  free-stream L(const) = 0; conservation on periodic domains; face term by 24-point quadrature
+ *   C6+C7  Keplerian equilibrium residual -> 0 at rate h^(p+1)
+ *   C8  y' = lambda y observed order 2 / 3; exact on polynomials of degree <= order
+ *   C7+C8  isentropic-vortex L1 error slope ~ p+1
+ *   C10 hand value on a constant state;  C11 R = 0 identity, fixed point, tau -> 0 limit
+ *   absolute per-step values: PARITY UNPINNED (paper prints none).
+ */
+#include "ref_dg.h"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+const int MAXM = 5;
+const int NV = 4;                         /* rho, rho vx, rho vy, E */
+
+struct Tables {
+  int m;
+  double xi[MAXM], w[MAXM];
+  double B[MAXM][MAXM];                   /* B[q][a] = phi_a(xi_q)   */
+  double D[MAXM][MAXM];                   /* D[q][a] = phi_a'(xi_q)  */
+  double Ep[MAXM], Em[MAXM];              /* phi_a(+1), phi_a(-1)    */
+};
+
+/* Legendre P_n(x) and P_n'(x) by the three-term recurrence. */
+void legendre(int n, double x, double* P, double* dP) {
+  double p0 = 1.0, p1 = x, d0 = 0.0, d1 = 1.0;
+  if (n == 0) { *P = p0; *dP = d0; return; }
+  for (int k = 2; k <= n; ++k) {
+    double pk = ((2.0 * k - 1.0) * x * p1 - (k - 1.0) * p0) / k;
+    double dk = d0 + (2.0 * k - 1.0) * p1;          /* P_k' = P_{k-2}' + (2k-1) P_{k-1} */
+    p0 = p1; p1 = pk; d0 = d1; d1 = dk;
+  }
+  *P = p1; *dP = d1;
+}
+
+/* C1 */
+void build_tables(int m, Tables* T) {
+  T->m = m;
+  const double pi = 3.14159265358979323846;
+  for (int q = 0; q < m; ++q) {
+    /* Newton iteration on P_m from the Chebyshev guess; nodes in ascending order */
+    double x = -std::cos(pi * (q + 0.75) / (m + 0.5));
+    for (int it = 0; it < 100; ++it) {
+      double P, dP;
+      legendre(m, x, &P, &dP);
+      double dx = P / dP;
+      x -= dx;
+      if (std::fabs(dx) < 1e-16) break;
+    }
+    double P, dP;
+    legendre(m, x, &P, &dP);
+    T->xi[q] = x;
+    T->w[q] = 2.0 / ((1.0 - x * x) * dP * dP);
+  }
+  if (m % 2 == 1) T->xi[m / 2] = 0.0;
+  for (int q = 0; q < m; ++q)
+    for (int a = 0; a < m; ++a) {
+      double P, dP;
+      legendre(a, T->xi[q], &P, &dP);
+      double s = std::sqrt(2.0 * a + 1.0);
+      T->B[q][a] = s * P;
+      T->D[q][a] = s * dP;
+    }
+  for (int a = 0; a < m; ++a) {
+    double s = std::sqrt(2.0 * a + 1.0);
+    T->Ep[a] = s;
+    T->Em[a] = (a % 2 == 0) ? s : -s;
+  }
+}
+
+/* C4: sound speed squared of the locally isothermal closure at (x,y). */
+inline double cs2_iso(const ref_params& p, double x, double y) {
+  return p.h_aspect * p.h_aspect * p.gm_star / std::sqrt(x * x + y * y + p.eps_star * p.eps_star);
+}
+
+/* C3 + C4: flux in direction dir of the state U at the point (x,y); also v_n and c. */
+void point_flux(const ref_params& p, const double* U, double x, double y, int dir,
+                double* F, double* vn, double* c) {
+  const double rho = U[0], mx = U[1], my = U[2], E = U[3];
+  const double vx = mx / rho, vy = my / rho;
+  double pr, cc;
+  if (p.eos == 0) {
+    pr = (p.gamma - 1.0) * (E - 0.5 * (mx * mx + my * my) / rho);
+    cc = std::sqrt(p.gamma * pr / rho);
+  } else {
+    const double cs2 = cs2_iso(p, x, y);
+    pr = cs2 * rho;
+    cc = std::sqrt(cs2);
+  }
+  if (dir == 0) {
+    F[0] = mx; F[1] = mx * vx + pr; F[2] = my * vx; F[3] = (E + pr) * vx; *vn = vx;
+  } else {
+    F[0] = my; F[1] = mx * vy; F[2] = my * vy + pr; F[3] = (E + pr) * vy; *vn = vy;
+  }
+  *c = cc;
+}
+
+/* C5 */
+void llf(const ref_params& p, const double* UL, const double* UR, double x, double y, int dir,
+         double* H) {
+  double FL[NV], FR[NV], vL, vR, cL, cR;
+  point_flux(p, UL, x, y, dir, FL, &vL, &cL);
+  point_flux(p, UR, x, y, dir, FR, &vR, &cR);
+  const double lam = std::fmax(std::fabs(vL) + cL, std::fabs(vR) + cR);
+  for (int v = 0; v < NV; ++v) H[v] = 0.5 * (FL[v] + FR[v]) - 0.5 * lam * (UR[v] - UL[v]);
+}
+
+/* C6 */
+void gravity(const ref_params& p, double t, double x, double y, double* g) {
+  g[0] = 0.0; g[1] = 0.0;
+  if (p.gm_star == 0.0) return;
+  {
+    const double r2 = x * x + y * y + p.eps_star * p.eps_star;
+    const double r3 = r2 * std::sqrt(r2);
+    g[0] -= p.gm_star * x / r3;
+    g[1] -= p.gm_star * y / r3;
+  }
+  if (p.q_planet != 0.0) {
+    const double ang = p.omega_planet * t + p.phase0;
+    const double xp = p.r_planet * std::cos(ang), yp = p.r_planet * std::sin(ang);
+    const double dx = x - xp, dy = y - yp;
+    const double r2 = dx * dx + dy * dy + p.eps_planet * p.eps_planet;
+    const double r3 = r2 * std::sqrt(r2);
+    g[0] -= p.q_planet * p.gm_star * dx / r3;
+    g[1] -= p.q_planet * p.gm_star * dy / r3;
+  }
+}
+
+}  // namespace
+
+struct ref_ctx {
+  ref_params p;
+  Tables T;
+  int m;
+  long ncoef;                 /* ny*nx*4*m*m */
+  double dx, dy, t;
+  bool has_state;
+  std::vector<double> U, U0;
+};
+
+namespace {
+
+inline long cell_off(const ref_ctx* c, int i, int j) { return ((long)j * c->p.nx + i) * NV * c->m * c->m; }
+
+/* trace of the polynomial of cell (i,j) in array A at xi = side (x-faces, function of eta_r)
+ * or eta = side (y-faces, function of xi_q):  U(+-1, eta_r) = sum_b sum_a A_ab E[a] B[r][b]. */
+void trace_x(const ref_ctx* c, const double* A, int i, int j, int side, int r, double* out) {
+  const int m = c->m;
+  const double* E = side > 0 ? c->T.Ep : c->T.Em;
+  const double* a0 = A + cell_off(c, i, j);
+  for (int v = 0; v < NV; ++v) {
+    double s = 0.0;
+    for (int b = 0; b < m; ++b)
+      for (int a = 0; a < m; ++a) s += a0[(v * m + b) * m + a] * E[a] * c->T.B[r][b];
+    out[v] = s;
+  }
+}
+void trace_y(const ref_ctx* c, const double* A, int i, int j, int side, int q, double* out) {
+  const int m = c->m;
+  const double* E = side > 0 ? c->T.Ep : c->T.Em;
+  const double* a0 = A + cell_off(c, i, j);
+  for (int v = 0; v < NV; ++v) {
+    double s = 0.0;
+    for (int b = 0; b < m; ++b)
+      for (int a = 0; a < m; ++a) s += a0[(v * m + b) * m + a] * c->T.B[q][a] * E[b];
+    out[v] = s;
+  }
+}
+
+/* C7 (with C2, C3, C5, C6, C9).  parts: 1 volume flux, 2 faces, 4 source. */
+void compute_rhs(const ref_ctx* c, const double* U, double t, int parts, double* L) {
+  const ref_params& p = c->p;
+  const Tables& T = c->T;
+  const int m = c->m, nx = p.nx, ny = p.ny;
+  const double dx = c->dx, dy = c->dy;
+
+  /* numerical fluxes on all x-faces [j][f][r][v], f = 0..nx, and y-faces [f][i][q][v], f = 0..ny */
+  std::vector<double> HX((size_t)ny * (nx + 1) * m * NV, 0.0), HY((size_t)(ny + 1) * nx * m * NV, 0.0);
+  if (parts & 2) {
+#pragma omp parallel for schedule(static)
+    for (int j = 0; j < ny; ++j)
+      for (int f = 0; f <= nx; ++f)
+        for (int r = 0; r < m; ++r) {
+          double UL[NV], UR[NV];
+          const double xf = p.x0 + f * dx;
+          const double yr = p.y0 + (j + 0.5) * dy + 0.5 * dy * T.xi[r];
+          if (f > 0 && f < nx) {
+            trace_x(c, U, f - 1, j, +1, r, UL);
+            trace_x(c, U, f, j, -1, r, UR);
+          } else if (p.bc == 0) {                       /* C9 periodic: wrap */
+            trace_x(c, U, nx - 1, j, +1, r, UL);
+            trace_x(c, U, 0, j, -1, r, UR);
+          } else if (f == 0) {
+            trace_x(c, U, 0, j, -1, r, UR);
+            if (p.bc == 1) std::memcpy(UL, UR, sizeof UL);           /* transmissive */
+            else trace_x(c, c->U0.data(), 0, j, -1, r, UL);            /* frozen to initial */
+          } else {
+            trace_x(c, U, nx - 1, j, +1, r, UL);
+            if (p.bc == 1) std::memcpy(UR, UL, sizeof UR);
+            else trace_x(c, c->U0.data(), nx - 1, j, +1, r, UR);
+          }
+          llf(p, UL, UR, xf, yr, 0, &HX[(((size_t)j * (nx + 1) + f) * m + r) * NV]);
+        }
+#pragma omp parallel for schedule(static)
+    for (int f = 0; f <= ny; ++f)
+      for (int i = 0; i < nx; ++i)
+        for (int q = 0; q < m; ++q) {
+          double UL[NV], UR[NV];
+          const double yf = p.y0 + f * dy;
+          const double xq = p.x0 + (i + 0.5) * dx + 0.5 * dx * T.xi[q];
+          if (f > 0 && f < ny) {
+            trace_y(c, U, i, f - 1, +1, q, UL);
+            trace_y(c, U, i, f, -1, q, UR);
+          } else if (p.bc == 0) {
+            trace_y(c, U, i, ny - 1, +1, q, UL);
+            trace_y(c, U, i, 0, -1, q, UR);
+          } else if (f == 0) {
+            trace_y(c, U, i, 0, -1, q, UR);
+            if (p.bc == 1) std::memcpy(UL, UR, sizeof UL);
+            else trace_y(c, c->U0.data(), i, 0, -1, q, UL);
+          } else {
+            trace_y(c, U, i, ny - 1, +1, q, UL);
+            if (p.bc == 1) std::memcpy(UR, UL, sizeof UR);
+            else trace_y(c, c->U0.data(), i, ny - 1, +1, q, UR);
+          }
+          llf(p, UL, UR, xq, yf, 1, &HY[(((size_t)f * nx + i) * m + q) * NV]);
+        }
+  }
+
+#pragma omp parallel for schedule(static)
+  for (int j = 0; j < ny; ++j)
+    for (int i = 0; i < nx; ++i) {
+      const double* u = U + cell_off(c, i, j);
+      double* Lc = L + cell_off(c, i, j);
+      const double xc = p.x0 + (i + 0.5) * dx, yc = p.y0 + (j + 0.5) * dy;
+      /* C2: nodal values at the m x m Gauss-Legendre points; C3: F, G; C6: S */
+      double Fq[MAXM][MAXM][NV], Gq[MAXM][MAXM][NV], Sq[MAXM][MAXM][NV];
+      for (int r = 0; r < m; ++r)
+        for (int q = 0; q < m; ++q) {
+          double Un[NV];
+          for (int v = 0; v < NV; ++v) {
+            double s = 0.0;
+            for (int b = 0; b < m; ++b)
+              for (int a = 0; a < m; ++a) s += u[(v * m + b) * m + a] * T.B[q][a] * T.B[r][b];
+            Un[v] = s;
+          }
+          const double x = xc + 0.5 * dx * T.xi[q], y = yc + 0.5 * dy * T.xi[r];
+          double vn, cc;
+          point_flux(p, Un, x, y, 0, Fq[q][r], &vn, &cc);
+          point_flux(p, Un, x, y, 1, Gq[q][r], &vn, &cc);
+          double g[2];
+          gravity(p, t, x, y, g);
+          Sq[q][r][0] = 0.0;
+          Sq[q][r][1] = Un[0] * g[0];
+          Sq[q][r][2] = Un[0] * g[1];
+          Sq[q][r][3] = Un[1] * g[0] + Un[2] * g[1];
+        }
+      for (int v = 0; v < NV; ++v)
+        for (int b = 0; b < m; ++b)
+          for (int a = 0; a < m; ++a) {
+            double vol = 0.0, src = 0.0, fx = 0.0, fy = 0.0;
+            for (int q = 0; q < m; ++q)
+              for (int r = 0; r < m; ++r) {
+                const double ww = T.w[q] * T.w[r];
+                vol += ww * ((2.0 / dx) * Fq[q][r][v] * T.D[q][a] * T.B[r][b] +
+                             (2.0 / dy) * Gq[q][r][v] * T.B[q][a] * T.D[r][b]);
+                src += ww * Sq[q][r][v] * T.B[q][a] * T.B[r][b];
+              }
+            if (parts & 2) {
+              for (int r = 0; r < m; ++r) {
+                const double hE = HX[(((size_t)j * (nx + 1) + i + 1) * m + r) * NV + v];
+                const double hW = HX[(((size_t)j * (nx + 1) + i) * m + r) * NV + v];
+                fx += T.w[r] * (hE * T.Ep[a] - hW * T.Em[a]) * T.B[r][b];
+              }
+              for (int q = 0; q < m; ++q) {
+                const double hN = HY[(((size_t)(j + 1) * nx + i) * m + q) * NV + v];
+                const double hS = HY[(((size_t)j * nx + i) * m + q) * NV + v];
+                fy += T.w[q] * (hN * T.Ep[b] - hS * T.Em[b]) * T.B[q][a];
+              }
+            }
+            double acc = 0.0;
+            if (parts & 1) acc += 0.25 * vol;
+            if (parts & 4) acc += 0.25 * src;
+            if (parts & 2) acc += -fx / (2.0 * dx) - fy / (2.0 * dy);
+            Lc[(v * m + b) * m + a] = acc;
+          }
+    }
+}
+
+struct RhsClosure { const ref_ctx* c; };
+void dg_ode(void* user, double t, const double* y, double* dydt) {
+  compute_rhs(static_cast<RhsClosure*>(user)->c, y, t, 7, dydt);
+}
+
+/* C11 */
+void damp(ref_ctx* c, double dt) {
+  const ref_params& p = c->p;
+  if (!(p.damp_r0 > 0.0)) return;
+  const int m = c->m;
+  const double pi = 3.14159265358979323846;
+  for (int j = 0; j < p.ny; ++j)
+    for (int i = 0; i < p.nx; ++i) {
+      const double xc = p.x0 + (i + 0.5) * c->dx, yc = p.y0 + (j + 0.5) * c->dy;
+      const double r = std::sqrt(xc * xc + yc * yc);
+      if (!(r > p.damp_r0)) continue;
+      double s = (r - p.damp_r0) / (p.damp_r1 - p.damp_r0);
+      double R = s * s;
+      if (R > 1.0) R = 1.0;
+      if (!(R > 0.0)) continue;
+      const double tau = 2.0 * pi * std::sqrt(p.damp_r0 * p.damp_r0 * p.damp_r0 / p.gm_star) / R;
+      double* u = c->U.data() + cell_off(c, i, j);
+      const double* u0 = c->U0.data() + cell_off(c, i, j);
+      for (int k = 0; k < NV * m * m; ++k) u[k] = (dt * u0[k] + tau * u[k]) / (tau + dt);
+    }
+}
+
+int check_params(const ref_params* p) {
+  if (!p) return -1;
+  if (p->nx < 1 || p->ny < 1 || p->order < 1 || p->order > MAXM) return -1;
+  if (!(p->x1 > p->x0) || !(p->y1 > p->y0)) return -1;
+  if (p->rk != 2 && p->rk != 3) return -1;
+  if (p->bc < 0 || p->bc > 2 || p->eos < 0 || p->eos > 1) return -1;
+  if (p->eos == 0 && !(p->gamma > 1.0)) return -1;
+  if (p->eos == 1 && !(p->h_aspect > 0.0 && p->gm_star > 0.0)) return -1;
+  if (p->damp_r0 > 0.0 && !(p->damp_r1 > p->damp_r0 && p->gm_star > 0.0)) return -1;
+  return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ref_init(const ref_params* p, ref_ctx** out) {
+  if (!out || check_params(p) != 0) return -1;
+  ref_ctx* c = new ref_ctx;
+  c->p = *p;
+  c->m = p->order;
+  build_tables(c->m, &c->T);
+  c->ncoef = (long)p->ny * p->nx * NV * c->m * c->m;
+  c->dx = (p->x1 - p->x0) / p->nx;
+  c->dy = (p->y1 - p->y0) / p->ny;
+  c->t = p->t0;
+  c->has_state = false;
+  *out = c;
+  return 0;
+}
+
+int ref_set_state(ref_ctx* c, const double* U) {
+  if (!c || !U) return -1;
+  c->U.assign(U, U + c->ncoef);
+  c->U0 = c->U;
+  c->has_state = true;
+  return 0;
+}
+
+int ref_get_state(ref_ctx* c, double* U) {
+  if (!c || !U || !c->has_state) return -1;
+  std::memcpy(U, c->U.data(), sizeof(double) * c->ncoef);
+  return 0;
+}
+
+int ref_rhs(ref_ctx* c, double t, double* L) { return ref_rhs_parts(c, t, 7, L); }
+
+int ref_rhs_parts(ref_ctx* c, double t, int parts, double* L) {
+  if (!c || !L || !c->has_state) return -1;
+  compute_rhs(c, c->U.data(), t, parts, L);
+  return 0;
+}
+
+/* C10 */
+int ref_cfl_dt(ref_ctx* c, double cfl, double* dt) {
+  if (!c || !dt || !c->has_state) return -1;
+  const ref_params& p = c->p;
+  const int m = c->m;
+  double worst = 0.0;
+  for (int j = 0; j < p.ny; ++j)
+    for (int i = 0; i < p.nx; ++i) {
+      const double* u = c->U.data() + cell_off(c, i, j);
+      const double rho = u[0 * m * m], mx = u[1 * m * m], my = u[2 * m * m], E = u[3 * m * m];
+      const double vx = mx / rho, vy = my / rho;
+      double cs;
+      if (p.eos == 0) {
+        const double pr = (p.gamma - 1.0) * (E - 0.5 * (mx * mx + my * my) / rho);
+        cs = std::sqrt(p.gamma * pr / rho);
+      } else {
+        const double xc = p.x0 + (i + 0.5) * c->dx, yc = p.y0 + (j + 0.5) * c->dy;
+        cs = std::sqrt(cs2_iso(p, xc, yc));
+      }
+      const double s = (std::fabs(vx) + cs) / c->dx + (std::fabs(vy) + cs) / c->dy;
+      if (s > worst) worst = s;
+    }
+  *dt = cfl / (2.0 * (m - 1) + 1.0) / worst;
+  return 0;
+}
+
+/* C8: Shu-Osher form of SSP(2,2) and SSP(3,3) (Gottlieb & Shu 1998).
+ * Stage times c = (0,1) and (0,1,1/2). */
+int ref_rk_step(int rk, long n, double* y, double t, double dt, ref_ode_fn f, void* user,
+                double* stages) {
+  if (rk != 2 && rk != 3) return -1;
+  std::vector<double> L(n), u1(n), u2(n);
+  f(user, t, y, L.data());
+  for (long k = 0; k < n; ++k) u1[k] = y[k] + dt * L[k];
+  if (stages) std::memcpy(stages, u1.data(), sizeof(double) * n);
+  f(user, t + dt, u1.data(), L.data());
+  if (rk == 2) {
+    for (long k = 0; k < n; ++k) y[k] = 0.5 * y[k] + 0.5 * (u1[k] + dt * L[k]);
+    if (stages) std::memcpy(stages + n, y, sizeof(double) * n);
+    return 0;
+  }
+  for (long k = 0; k < n; ++k) u2[k] = 0.75 * y[k] + 0.25 * (u1[k] + dt * L[k]);
+  if (stages) std::memcpy(stages + n, u2.data(), sizeof(double) * n);
+  f(user, t + 0.5 * dt, u2.data(), L.data());
+  for (long k = 0; k < n; ++k) y[k] = (1.0 / 3.0) * y[k] + (2.0 / 3.0) * (u2[k] + dt * L[k]);
+  if (stages) std::memcpy(stages + 2 * n, y, sizeof(double) * n);
+  return 0;
+}
+
+int ref_step_debug(ref_ctx* c, double dt, double* stages) {
+  if (!c || !c->has_state) return -1;
+  RhsClosure cl{c};
+  int e = ref_rk_step(c->p.rk, c->ncoef, c->U.data(), c->t, dt, dg_ode, &cl, stages);
+  if (e) return e;
+  damp(c, dt);
+  c->t += dt;
+  return 0;
+}
+
+int ref_step(ref_ctx* c, double dt) { return ref_step_debug(c, dt, nullptr); }
+
+int ref_damp(ref_ctx* c, double dt) {
+  if (!c || !c->has_state) return -1;
+  damp(c, dt);
+  return 0;
+}
+
+double ref_time(const ref_ctx* c) { return c ? c->t : 0.0; }
+int ref_set_time(ref_ctx* c, double t) { if (!c) return -1; c->t = t; return 0; }
+void ref_destroy(ref_ctx* c) { delete c; }
+
+int ref_tables(int m, double* xi, double* w, double* B, double* D, double* Ep, double* Em) {
+  if (m < 1 || m > MAXM) return -1;
+  Tables T;
+  build_tables(m, &T);
+  for (int q = 0; q < m; ++q) {
+    xi[q] = T.xi[q]; w[q] = T.w[q]; Ep[q] = T.Ep[q]; Em[q] = T.Em[q];
+    for (int a = 0; a < m; ++a) { B[q * m + a] = T.B[q][a]; D[q * m + a] = T.D[q][a]; }
+  }
+  return 0;
+}
+
+int ref_point_flux(const ref_params* p, const double* U4, double x, double y, int dir,
+                   double* F4, double* vn, double* c) {
+  if (!p || (dir != 0 && dir != 1)) return -1;
+  point_flux(*p, U4, x, y, dir, F4, vn, c);
+  return 0;
+}
+
+int ref_llf(const ref_params* p, const double* UL, const double* UR, double x, double y, int dir,
+            double* H4) {
+  if (!p || (dir != 0 && dir != 1)) return -1;
+  llf(*p, UL, UR, x, y, dir, H4);
+  return 0;
+}
+
+int ref_gravity(const ref_params* p, double t, double x, double y, double* g2) {
+  if (!p) return -1;
+  gravity(*p, t, x, y, g2);
+  return 0;
+}
+
+int ref_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+void ref_set_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
+}  // extern "C"

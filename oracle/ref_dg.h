@@ -1,0 +1,77 @@
+/* CPU ORACLE -- TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * Plain, slow, single-threaded (optionally one `omp parallel for` over cell rows) fp64 restatement
+ * of the explicit modal DG right-hand side + SSP-RK stage update of arXiv:1805.01443 for the 2D
+ * Euler equations, written step by step in the paper's order and notation (SURVEY.md section 8(c),
+ * items C1..C11).  Host pointers only.  Shares no code, header, table or constant generator with
+ * the CUDA path (paper_1805_01443_b200/csrc, include/dg.h); neither includes the other.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * load this library.
+ *
+ * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): see the header of ref_dg.cpp.
+ * Absolute per-step numbers: PARITY UNPINNED (the paper prints none for this path, Fig. 2
+ * is an image) -- every other function below is pinned.
+ */
+#ifndef REF_DG_H
+#define REF_DG_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ref_ctx ref_ctx;
+
+typedef struct {
+  int32_t nx, ny;            /* uniform Cartesian grid of rectangles K_ij */
+  double  x0, x1, y0, y1;
+  int32_t order;             /* m = N_p + 1 = 1..5 */
+  int32_t rk;                /* 2: SSP(2,2), 3: SSP(3,3) */
+  int32_t bc;                /* 0 periodic, 1 transmissive, 2 frozen to the initial state */
+  int32_t eos;               /* 0 ideal gas p=(gamma-1)e; 1 locally isothermal */
+  double  gamma;
+  double  h_aspect;          /* eos 1: c_s^2 = h^2 GM / sqrt(r^2 + eps_star^2) */
+  double  gm_star, eps_star; /* softened star potential; gm_star = 0: no gravity at all */
+  double  q_planet, r_planet, eps_planet, omega_planet, phase0; /* planet on a fixed circular orbit */
+  double  damp_r0, damp_r1;  /* wave-killing zone r0 < r; r0 <= 0: off */
+  double  t0;
+} ref_params;
+
+/* --- the same surface as include/dg.h, prefixed ref_, host memory --- */
+int    ref_init(const ref_params* p, ref_ctx** out);
+int    ref_set_state(ref_ctx*, const double* U);   /* [ny][nx][4][m][m], snapshots U0 */
+int    ref_get_state(ref_ctx*, double* U);
+int    ref_rhs(ref_ctx*, double t, double* L);     /* L(u) of Eq.(3) divided by the mass, at time t */
+int    ref_cfl_dt(ref_ctx*, double cfl, double* dt);
+int    ref_step(ref_ctx*, double dt);              /* RK step (C8) + damping (C11); t += dt */
+int    ref_step_debug(ref_ctx*, double dt, double* stages); /* also u^(1..k), before damping */
+double ref_time(const ref_ctx*);
+int    ref_set_time(ref_ctx*, double t);
+void   ref_destroy(ref_ctx*);
+
+/* --- pieces exposed so that tests can pin them one by one --- */
+/* C1: Gauss-Legendre nodes/weights and the basis tables; arrays sized m, m, m*m, m*m, m, m. */
+int  ref_tables(int m, double* xi, double* w, double* B, double* D, double* Eplus, double* Eminus);
+/* C3/C4: physical flux in direction dir (0:x, 1:y) at point (x,y); returns normal velocity and c. */
+int  ref_point_flux(const ref_params*, const double* U4, double x, double y, int dir,
+                    double* F4, double* vn, double* c);
+/* C5: local Lax-Friedrichs flux across a face with normal +dir, left state UL, right state UR. */
+int  ref_llf(const ref_params*, const double* UL, const double* UR, double x, double y, int dir,
+             double* H4);
+/* C6: gravitational acceleration g = -grad Phi at (x,y), time t. */
+int  ref_gravity(const ref_params*, double t, double x, double y, double* g2);
+/* C7 split: parts bitmask 1 = volume flux term, 2 = face term, 4 = source term. */
+int  ref_rhs_parts(ref_ctx*, double t, int parts, double* L);
+/* C11 alone. */
+int  ref_damp(ref_ctx*, double dt);
+/* C8 alone: one RK step of y' = f(t,y) for n unknowns; stages (nullable) receives y^(1..k). */
+typedef void (*ref_ode_fn)(void* user, double t, const double* y, double* dydt);
+int  ref_rk_step(int rk, long n, double* y, double t, double dt, ref_ode_fn f, void* user,
+                 double* stages);
+/* number of OpenMP threads the library will use (1 if built without -fopenmp) */
+int  ref_threads(void);
+void ref_set_threads(int n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

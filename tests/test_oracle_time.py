@@ -1,0 +1,212 @@
+"""Pins for oracle C8 (SSP-RK), C10 (CFL), C11 (wave
+damping) and the end-to-end convergence order on the isentropic vortex
+(PAPER.md:181-215)."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1805_01443_b200 import workloads as W
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _tableaus():
+    d = {}
+    for line in open(os.path.join(GOLD, "rk_tableaus.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, kind, *v = line.split()
+        d[(name, kind)] = np.array([float(x) for x in v])
+    return d
+
+
+@pytest.mark.parametrize("rk", [2, 3])
+def test_rk_matches_butcher_tableau_on_time_only_rhs(rk):
+    """y' = f(t): one step must equal dt * sum_i b_i f(t + c_i dt) with the textbook (c, b) of
+    SSP(2,2) / SSP(3,3).  Pins the stage times (reading G8) and the weights."""
+    tb = _tableaus()
+    c, b = tb[(f"ssp{rk}{rk}", "c")], tb[(f"ssp{rk}{rk}", "b")]
+    assert abs(b.sum() - 1.0) < 1e-15
+    f = lambda t, y: np.array([math.exp(0.7 * t) + t ** 3])
+    t0, dt = 0.3, 0.11
+    y = oracle.rk_step(rk, np.array([2.0]), t0, dt, f)
+    ref = 2.0 + dt * sum(bi * f(t0 + ci * dt, None)[0] for bi, ci in zip(b, c))
+    assert abs(y[0] - ref) < 1e-15
+
+
+@pytest.mark.parametrize("rk", [2, 3])
+def test_rk_observed_order_on_linear_ode(rk):
+    lam = -1.3 + 0.4j
+
+    def f(t, y):
+        z = lam * (y[0] + 1j * y[1])
+        return np.array([z.real, z.imag])
+
+    errs = []
+    for n in (8, 16, 32):
+        y = np.array([1.0, 0.0])
+        dt = 1.0 / n
+        for k in range(n):
+            y = oracle.rk_step(rk, y, k * dt, dt, f)
+        errs.append(abs(y[0] + 1j * y[1] - np.exp(lam)))
+    rates = [math.log2(errs[i] / errs[i + 1]) for i in range(2)]
+    assert abs(rates[-1] - rk) < 0.15, rates
+    # amplification factor of one step is the degree-rk Taylor polynomial of exp(z)
+    z = lam * 0.25
+    y = oracle.rk_step(rk, np.array([1.0, 0.0]), 0.0, 0.25, f)
+    taylor = sum(z ** k / math.factorial(k) for k in range(rk + 1))
+    assert abs(y[0] + 1j * y[1] - taylor) < 1e-15
+
+
+@pytest.mark.parametrize("rk", [2, 3])
+def test_rk_stages_are_convex_combinations(rk):
+    """Shu-Osher form: every stage is a convex combination of forward-Euler steps."""
+    f = lambda t, y: -2.0 * y
+    y0 = np.array([1.0, -3.0])
+    dt = 0.1
+    y, st = oracle.rk_step(rk, y0, 0.0, dt, f, want_stages=True)
+    fe = lambda u: u + dt * f(0, u)
+    np.testing.assert_allclose(st[0], fe(y0), rtol=1e-15)
+    if rk == 2:
+        np.testing.assert_allclose(st[1], 0.5 * y0 + 0.5 * fe(st[0]), rtol=1e-15)
+    else:
+        np.testing.assert_allclose(st[1], 0.75 * y0 + 0.25 * fe(st[0]), rtol=1e-15)
+        np.testing.assert_allclose(st[2], y0 / 3 + 2 / 3 * fe(st[1]), rtol=1e-15)
+    np.testing.assert_array_equal(st[-1], y)
+
+
+def test_dg_step_uses_stage_times_for_the_planet():
+    """Two oracles started at t0 and t0+T_planet give identical steps; shifting by half a period
+    does not: the source is evaluated at the running stage time."""
+    p, U = W.random_smooth(4, 4, 2, seed=4, gravity=True, rk=3)
+    T = 2 * math.pi / p["omega_planet"]
+    outs = []
+    for t0 in (0.0, T, 0.5 * T):
+        r = oracle.RefDG(dict(p, t0=t0))
+        r.set_state(U)
+        r.step(0.01)
+        outs.append(r.get_state())
+    np.testing.assert_allclose(outs[0], outs[1], rtol=0, atol=1e-13)
+    assert np.abs(outs[0] - outs[2]).max() > 1e-7
+
+
+@pytest.mark.parametrize("m", [1, 3, 5])
+def test_cfl_hand_value_constant_state(m):
+    """dt = C/(2p+1) * dx / (|vx| + |vy| + 2c) for dx = dy."""
+    n = 7
+    p = W.make_params(nx=n, ny=n, order=m, x0=0.0, x1=3.5, y0=0.0, y1=3.5, eos=0, gamma=1.4)
+    rho, vx, vy, pr = 2.0, 3.0, -1.0, 4.0
+    U = np.zeros((n, n, 4, m, m))
+    U[..., 0, 0] = [rho, rho * vx, rho * vy, pr / 0.4 + 0.5 * rho * (vx * vx + vy * vy)]
+    r = oracle.RefDG(p)
+    r.set_state(U)
+    ref = 0.2 / (2 * (m - 1) + 1) * 0.5 / (abs(vx) + abs(vy) + 2 * math.sqrt(1.4 * pr / rho))
+    assert abs(r.cfl_dt(0.2) - ref) < 1e-16
+    # only the zeroth modes enter: junk in higher modes changes nothing
+    if m > 1:
+        U[..., 1, 1] = 0.3
+        r.set_state(U)
+        assert abs(r.cfl_dt(0.2) - ref) < 1e-16
+
+
+def test_cfl_isothermal_uses_cell_centre_sound_speed():
+    n, m = 4, 2
+    p = W.make_params(nx=n, ny=n, order=m, x0=1.0, x1=2.0, y0=1.0, y1=2.0, eos=1, h_aspect=0.1,
+                      gm_star=1.0, eps_star=0.0)
+    U = np.zeros((n, n, 4, m, m))
+    U[..., 0, 0] = [1.0, 0.0, 0.0, 1.0]
+    r = oracle.RefDG(p)
+    r.set_state(U)
+    # fastest cell is the one closest to the star: centre (1.125, 1.125)
+    c = math.sqrt(0.01 / math.hypot(1.125, 1.125))
+    assert abs(r.cfl_dt(0.3) - 0.3 / 3 * 0.25 / (2 * c)) < 1e-15
+
+
+def test_damping_properties():
+    p, U = W.disc(16, 2, planet=False)
+    r = oracle.RefDG(p)
+    r.set_state(U)
+    r.damp(0.1)
+    np.testing.assert_allclose(r.get_state(), U, rtol=4e-16, atol=0)   # fixed point U = U0
+    # perturb everywhere, damp: cells with r <= r0 untouched, others relax towards U0
+    # (the snapshot is taken by set_state, so perturb through a second context sharing U0 = U)
+    r = oracle.RefDG(p)
+    r.set_state(U)
+    r.step(0.0)                                                 # zero-length step keeps U
+    np.testing.assert_allclose(r.get_state(), U, atol=1e-15)
+    h = 5.0 / 16
+    xc = -2.5 + (np.arange(16) + 0.5) * h
+    R = np.hypot(xc[None, :], xc[:, None])
+    # emulate a perturbed state with the same snapshot: run real steps, then damp separately
+    for _ in range(3):
+        r.step(r.cfl_dt(0.2))
+    before = r.get_state()
+    dt = 0.05
+    r.damp(dt)
+    after = r.get_state()
+    inside = R <= 2.2
+    np.testing.assert_array_equal(after[inside], before[inside])
+    ramp = np.minimum(1.0, ((R - 2.2) / 0.3) ** 2)
+    tau = 2 * math.pi * math.sqrt(2.2 ** 3) / np.where(ramp > 0, ramp, 1.0)
+    ref = (dt * U + tau[..., None, None, None] * before) / (tau[..., None, None, None] + dt)
+    np.testing.assert_allclose(after[~inside], ref[~inside], rtol=1e-14, atol=1e-18)
+    # dt >> tau limit: state -> U0 where R > 0
+    r.damp(1e12)
+    np.testing.assert_allclose(r.get_state()[~inside], U[~inside], rtol=1e-9)
+
+
+def test_step_debug_last_stage_is_new_state_without_damping():
+    p, U = W.vortex(8, 2)
+    r = oracle.RefDG(p)
+    r.set_state(U)
+    st = r.step_debug(0.01)
+    assert st.shape == (2,) + U.shape
+    np.testing.assert_array_equal(st[-1], r.get_state())
+    assert abs(r.time - 0.01) < 1e-18
+
+
+def _l1_density_error(p, U, exact_rho, T, fine=8):
+    """L1 density error in the spirit of Eq.(5), but with a `fine`-point rule per
+    cell and direction so that the polynomial between the nodes is measured too."""
+    from numpy.polynomial.legendre import leggauss, legval
+    m, n = p["order"], p["nx"]
+    r = oracle.RefDG(p, omp=True)
+    r.set_state(U)
+    while r.time < T - 1e-14:
+        r.step(min(r.cfl_dt(0.2), T - r.time))
+    xs, ws = leggauss(fine)
+    B = np.array([math.sqrt(2 * a + 1) * legval(xs, np.eye(m)[a]) for a in range(m)])
+    un = np.einsum("jiba,ax,by->jiyx", r.get_state()[:, :, 0], B, B)
+    h = (p["x1"] - p["x0"]) / n
+    xc = p["x0"] + (np.arange(n) + 0.5) * h
+    X = xc[None, :, None, None] + 0.5 * h * xs[None, None, None, :]
+    Y = xc[:, None, None, None] + 0.5 * h * xs[None, None, :, None]
+    err = np.abs(un - exact_rho(X, Y, r.time))
+    return 0.25 * h * h * (err * ws[None, None, :, None] * ws[None, None, None, :]).sum()
+
+
+@pytest.mark.parametrize("m,grids", [(2, (16, 32)), (3, (16, 32)), (4, (8, 16))])
+def test_entropy_wave_convergence_order(m, grids):
+    """Smooth exact Euler solution: observed L1 rate = N_p + 1."""
+    e = []
+    for n in grids:
+        p, U = W.entropy_wave(n, m, rk=3)
+        e.append(_l1_density_error(p, U, W.entropy_wave_exact, 0.25))
+    rate = math.log2(e[0] / e[1])
+    assert abs(rate - m) < 0.3, (e, rate)
+
+
+@pytest.mark.parametrize("m,rk,grids", [(2, 2, (10, 20)), (3, 3, (8, 16)), (4, 3, (8, 16)), (5, 3, (6, 12))])
+def test_vortex_convergence_order(m, rk, grids):
+    """Isentropic vortex: rate close to N_p + 1 on coarse grids, where the error
+    is far above the 2e-5 velocity kink of the periodic images (SURVEY 8(c) caveat).  Even N_p is
+    observed at N_p + 1/2 on this problem, hence the one-sided window."""
+    e = []
+    for n in grids:
+        p, U = W.vortex(n, m, rk=rk)
+        e.append(_l1_density_error(p, U, lambda X, Y, t: W.vortex_exact(X, Y, t)[0], 0.25))
+    rate = math.log2(e[0] / e[1])
+    assert m - 0.6 < rate < m + 1.7, (e, rate)
