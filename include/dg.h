@@ -1,0 +1,135 @@
+/* libdg -- C-ABI boundary of the B200 (sm_100a) discontinuous-Galerkin Euler hot path.
+ *
+ * Method: arXiv:1805.01443 ("Planet-disc interactions with Discontinuous Galerkin Methods using
+ * GPUs"), cited below as PAPER.md:<line> (the text under /root/reference at build time).
+ * One GPU, fp64, DG orders m = 1..5 (polynomial degree N_p = m-1), uniform Cartesian mesh.
+ *
+ * Conventions
+ * -----------
+ *  - Plain C: pointers and sizes only.  Every pointer argument is tagged DEVICE or HOST below.
+ *  - The library never allocates device memory: the caller passes a DEVICE workspace of at least
+ *    dg_workspace_bytes() bytes (256-byte aligned) to dg_init and keeps it alive until dg_destroy.
+ *    The library owns only the host-side context.
+ *  - All work is enqueued on the CUDA stream given to dg_init (a cudaStream_t passed as void*,
+ *    0 = legacy default stream).  Calls are asynchronous unless stated otherwise.
+ *  - External state layout (both directions), fp64, C order:
+ *        U[ny][nx][4][m][m]  =  U[j][i][v][b][a]
+ *    j,i cell indices (i along x, fastest of the two), v in {rho, rho*vx, rho*vy, E},
+ *    a = Legendre degree in x (fastest), b = degree in y, of the orthonormal tensor basis
+ *    phi_a(xi) phi_b(eta), phi_n = sqrt(2n+1) P_n on the reference square [-1,1]^2
+ *    (mode (0,0) is the cell average).
+ *    Inside the workspace the state lives in a different, kernel-friendly layout.
+ *  - Return value: 0 (DG_OK) or a negative DG_E* code; dg_last_error() gives a message.
+ *    No exceptions, no aborts, nothing is printed.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns DG_ECUDA.
+ */
+#ifndef DG_H
+#define DG_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DG_OK       0
+#define DG_EINVAL  (-1)   /* bad parameter, null or misaligned pointer */
+#define DG_ENOSPC  (-2)   /* workspace too small */
+#define DG_ESTATE  (-3)   /* state not set yet */
+#define DG_ECUDA   (-4)   /* CUDA runtime / launch error (message in dg_last_error) */
+
+typedef struct dg_ctx dg_ctx;     /* opaque, host-side, owned by the library */
+
+typedef struct {
+  int32_t nx, ny;                 /* cells K_ij = [x_{i-1/2},x_{i+1/2}] x [y_{j-1/2},y_{j+1/2}] */
+  double  x0, x1, y0, y1;         /* domain; dx = (x1-x0)/nx, dy = (y1-y0)/ny */
+  int32_t order;                  /* m = 1..5: m x m modes per cell and variable */
+  int32_t rk;                     /* 2: SSP-RK(2,2), 3: SSP-RK(3,3) (Gottlieb & Shu 1998) */
+  int32_t bc;                     /* 0 periodic; 1 transmissive (exterior trace = interior);
+                                     2 frozen: exterior trace = trace of the state given to the last
+                                     dg_set_state*, same boundary cell, same face point */
+  int32_t eos;                    /* 0 ideal gas p = (gamma-1) e, Eq.(2) PAPER.md:45-49;
+                                     1 locally isothermal p = c_s^2(x,y) rho (BASELINE.json configs 1-4) */
+  double  gamma;                  /* adiabatic index (eos 0) */
+  double  h_aspect;               /* eos 1: c_s^2 = h^2 GM / sqrt(x^2 + y^2 + eps_star^2) */
+  double  gm_star, eps_star;      /* star potential -GM/sqrt(r^2+eps^2); gm_star = 0: no gravity */
+  double  q_planet, r_planet, eps_planet, omega_planet, phase0;
+                                  /* planet of mass ratio q on the fixed circular orbit
+                                     r_p (cos, sin)(omega_p t + phase0), softening eps_p;
+                                     no indirect term; q = 0: no planet */
+  double  damp_r0, damp_r1;       /* wave-killing zone r0 < r (<= r1 and beyond); r0 <= 0: off */
+  double  t0;                     /* initial time */
+} dg_params;
+
+/* Bytes of DEVICE workspace dg_init needs for these parameters (0 if they are invalid). */
+size_t dg_workspace_bytes(const dg_params* params /*HOST*/);
+
+/* Create a context.  workspace: DEVICE, 256-byte aligned, >= dg_workspace_bytes(params) bytes,
+ * owned by the caller.  cuda_stream: cudaStream_t.  Builds the quadrature/basis tables
+ * on the host.  Errors: DG_EINVAL, DG_ENOSPC. */
+int dg_init(const dg_params* params /*HOST*/, void* workspace /*DEVICE*/, size_t workspace_bytes,
+            void* cuda_stream, dg_ctx** out /*HOST*/);
+
+/* Copy a modal state into the context (steps (i)(b)-(c) of PAPER.md:141-144 are the caller's).
+ * U: [ny][nx][4][m][m] doubles.  Also snapshots it as the "initial" state used by bc 2 and by the
+ * damping zones, and resets the time to t0.  _host variant: U is HOST memory (pinned memory makes
+ * the copy asynchronous); the host->device copy is enqueued on the stream. */
+int dg_set_state(dg_ctx*, const double* U /*DEVICE*/);
+int dg_set_state_host(dg_ctx*, const double* U /*HOST*/);
+
+/* Copy the current modal state out.  dg_get_state_host synchronises the stream before returning. */
+int dg_get_state(dg_ctx*, double* U /*DEVICE*/);
+int dg_get_state_host(dg_ctx*, double* U /*HOST*/);
+
+/* L(u) at time t: right-hand side of the semi-discrete form Eq.(3) divided by the
+ * diagonal mass: volume flux term + face term with the local Lax-Friedrichs
+ * numerical flux + gravity source.  L: [ny][nx][4][m][m] DEVICE.  The state is not changed. */
+int dg_rhs(dg_ctx*, double t, double* L /*DEVICE*/);
+
+/* Global time step:
+ *   dt = cfl/(2 N_p + 1) / max_K [ (|vx|+c)/dx + (|vy|+c)/dy ]   from the cell averages.
+ * Synchronises the stream (the only blocking call of the time loop) and writes one HOST double. */
+int dg_cfl_dt(dg_ctx*, double cfl, double* dt /*HOST*/);
+
+/* One full time step of size dt (Algorithm 1, in Shu-Osher form): rk stages of
+ * u^(s) = alpha_s u^n + beta_s (u^(s-1) + dt L(u^(s-1), t^n + c_s dt)), then the wave-killing
+ * relaxation Q <- (dt Q0 + tau Q)/(tau + dt) if enabled; t += dt. */
+int dg_step(dg_ctx*, double dt);
+
+/* Same, and also writes the rk stage states u^(1..k) (before damping), modal layout,
+ * stages: [rk][ny][nx][4][m][m] DEVICE.  For per-stage parity tests. */
+int dg_step_debug(dg_ctx*, double dt, double* stages /*DEVICE*/);
+
+/* Convenience for end-to-end runs from HOST buffers: set_state_host(U_in), then nsteps times
+ * { dg_cfl_dt(cfl); dg_step(dt) }, then get_state_host(U_out).  Blocking. */
+int dg_run_host(dg_ctx*, const double* U_in /*HOST*/, int nsteps, double cfl, double* U_out /*HOST*/);
+
+double dg_time(const dg_ctx*);
+int    dg_set_time(dg_ctx*, double t);
+
+/* Number of kernels this context has launched so far (for launch accounting in bench.py). */
+long long dg_launch_count(const dg_ctx*);
+
+/* Tuning knobs (all have defaults; DG_EINVAL on unknown key or bad value).
+ *   DG_TUNE_ROWS_PER_CTA : rows of cells one thread block marches over in the stage kernel
+ *   DG_TUNE_FUSED_CFL    : 1 = the last RK stage also reduces the CFL wave speed (default), 0 = separate kernel */
+#define DG_TUNE_ROWS_PER_CTA 1
+#define DG_TUNE_FUSED_CFL    2
+int dg_set_tuning(dg_ctx*, int key, int value);
+
+/* Average-duration probe: enqueue CUDA events around the stage kernels of the next dg_step calls.
+ * dg_stage_time_ms returns the mean stage-kernel time (ms) accumulated since the last reset and
+ * the number of launches measured (synchronises). */
+int dg_stage_timing(dg_ctx*, int enable);
+int dg_stage_time_ms(dg_ctx*, double* mean_ms /*HOST*/, long long* launches /*HOST*/);
+
+/* Diagnostic: sustained fp64 FMA throughput of this GPU (register-resident DFMA loop),
+ * TFLOP/s counting an FMA as 2 flops.  Uses the context's stream; blocking. */
+int dg_probe_fp64_peak(dg_ctx*, double* tflops /*HOST*/);
+
+const char* dg_last_error(const dg_ctx*);
+void dg_destroy(dg_ctx*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DG_H */

@@ -1,0 +1,524 @@
+// C-ABI of libdg (include/dg.h): host-side context, workspace carving, launch logic.
+// Everything numerical runs in the kernels of dg_kernels.cuh; there is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <type_traits>
+#include <vector>
+
+#include "../../include/dg.h"
+#include "dg_tables.h"
+#include "dg_kernels.cuh"
+
+using namespace dg;
+
+namespace {
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Layout {
+  int m, nbx;
+  size_t state_doubles;      // ny * nbx * 4 m^2 * 32
+  size_t state_bytes;
+  bool need_q0, need_btr;
+  size_t off_q[3], off_q0, off_btrW, off_btrE, off_btrS, off_btrN, off_scalars, total;
+};
+
+bool valid_params(const dg_params* p) {
+  if (!p) return false;
+  if (p->nx < 1 || p->ny < 1 || p->order < 1 || p->order > MAXM) return false;
+  if (!(p->x1 > p->x0) || !(p->y1 > p->y0)) return false;
+  if (p->rk != 2 && p->rk != 3) return false;
+  if (p->bc < 0 || p->bc > 2 || p->eos < 0 || p->eos > 1) return false;
+  if (p->eos == 0 && !(p->gamma > 1.0)) return false;
+  if (p->eos == 1 && !(p->h_aspect > 0.0 && p->gm_star > 0.0)) return false;
+  if (p->damp_r0 > 0.0 && !(p->damp_r1 > p->damp_r0 && p->gm_star > 0.0)) return false;
+  if (p->gm_star < 0.0 || p->q_planet < 0.0) return false;
+  return true;
+}
+
+Layout make_layout(const dg_params* p) {
+  Layout L{};
+  L.m = p->order;
+  L.nbx = (p->nx + 31) / 32;
+  L.state_doubles = (size_t)p->ny * L.nbx * 4 * L.m * L.m * 32;
+  L.state_bytes = align_up(L.state_doubles * sizeof(double));
+  L.need_q0 = p->bc == 2 || p->damp_r0 > 0.0;
+  L.need_btr = p->bc == 2;
+  size_t off = 0;
+  for (int k = 0; k < 3; ++k) { L.off_q[k] = off; off += L.state_bytes; }
+  L.off_q0 = off;
+  if (L.need_q0) off += L.state_bytes;
+  const size_t side = align_up((size_t)p->ny * 4 * L.m * sizeof(double));
+  const size_t top = align_up((size_t)L.nbx * 4 * L.m * 32 * sizeof(double));
+  L.off_btrW = off; if (L.need_btr) off += side;
+  L.off_btrE = off; if (L.need_btr) off += side;
+  L.off_btrS = off; if (L.need_btr) off += top;
+  L.off_btrN = off; if (L.need_btr) off += top;
+  L.off_scalars = off; off += ALIGN;
+  L.total = off;
+  return L;
+}
+}  // namespace
+
+struct dg_ctx {
+  dg_params p;
+  Layout L;
+  HostTables H;
+  DevTables T;
+  ConvTables CT;
+  Geom g;
+  cudaStream_t stream;
+  char* ws;
+  int cur;                    // index of the buffer holding u^n
+  bool has_state;
+  bool wmax_valid;            // the fused reduction of the last step matches the current state
+  double t;
+  int rows_per_cta;
+  int fused_cfl;
+  long long launches;
+  bool timing;
+  std::vector<cudaEvent_t> evs;      // pairs (start, stop) around stage kernels, recorded without syncing
+  size_t ev_used;
+  std::string err;
+
+  double* q(int k) const { return reinterpret_cast<double*>(ws + L.off_q[k]); }
+  double* q0() const { return reinterpret_cast<double*>(ws + L.off_q0); }
+  double* btrW() const { return reinterpret_cast<double*>(ws + L.off_btrW); }
+  double* btrE() const { return reinterpret_cast<double*>(ws + L.off_btrE); }
+  double* btrS() const { return reinterpret_cast<double*>(ws + L.off_btrS); }
+  double* btrN() const { return reinterpret_cast<double*>(ws + L.off_btrN); }
+  unsigned long long* wmax() const { return reinterpret_cast<unsigned long long*>(ws + L.off_scalars); }
+};
+
+namespace {
+
+int fail(dg_ctx* c, int code, const char* what, cudaError_t e = cudaSuccess) {
+  if (c) {
+    c->err = what;
+    if (e != cudaSuccess) { c->err += ": "; c->err += cudaGetErrorString(e); }
+  }
+  return code;
+}
+#define CUDA_TRY(c, call)                                            \
+  do {                                                               \
+    cudaError_t e_ = (call);                                         \
+    if (e_ != cudaSuccess) return fail((c), DG_ECUDA, #call, e_);    \
+  } while (0)
+
+Phys make_phys(const dg_ctx* c, double t) {
+  const dg_params& p = c->p;
+  Phys ph{};
+  ph.gamma = p.gamma;
+  ph.gm1 = p.gamma - 1.0;
+  ph.h2gm = p.h_aspect * p.h_aspect * p.gm_star;
+  ph.gm = p.gm_star;
+  ph.eps2s = p.eps_star * p.eps_star;
+  ph.qgm = p.q_planet * p.gm_star;
+  const double ang = p.omega_planet * t + p.phase0;
+  ph.xp = p.r_planet * std::cos(ang);
+  ph.yp = p.r_planet * std::sin(ang);
+  ph.eps2p = p.eps_planet * p.eps_planet;
+  return ph;
+}
+
+template <int M>
+int launch_stage_m(dg_ctx* c, const StageArgs& A) {
+  dim3 grid(c->L.nbx, (c->p.ny + A.rows - 1) / A.rows), block(M * 32);
+  if (c->p.eos == 0) stage_kernel<M, 0><<<grid, block, 0, c->stream>>>(A);
+  else               stage_kernel<M, 1><<<grid, block, 0, c->stream>>>(A);
+  return 0;
+}
+
+// One fused stage: qout = a*qn + b*(qprev + dt*L(qprev, t))  (or qout = L when rhs_only).
+int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout, double a, double b,
+                 double dt, double t, int flags) {
+  StageArgs A{};
+  A.qprev = qprev; A.qn = qn; A.qout = qout; A.q0 = c->q0();
+  A.btrW = c->btrW(); A.btrE = c->btrE(); A.btrS = c->btrS(); A.btrN = c->btrN();
+  A.wmax = c->wmax();
+  A.a = a; A.b = b; A.dt = dt;
+  A.damp_r0 = c->p.damp_r0;
+  A.damp_inv_w = c->p.damp_r0 > 0.0 ? 1.0 / (c->p.damp_r1 - c->p.damp_r0) : 0.0;
+  A.damp_tau0 = c->p.damp_r0 > 0.0
+      ? 2.0 * 3.14159265358979323846 * std::sqrt(c->p.damp_r0 * c->p.damp_r0 * c->p.damp_r0 / c->p.gm_star)
+      : 0.0;
+  A.rows = c->rows_per_cta;
+  if (c->p.gm_star > 0.0) flags |= F_GRAV;
+  if (c->p.gm_star > 0.0 && c->p.q_planet > 0.0) flags |= F_PLANET;
+  A.flags = flags;
+  A.g = c->g;
+  A.ph = make_phys(c, t);
+  A.T = c->T;
+  const bool timed = c->timing && c->ev_used + 2 <= c->evs.size();
+  if (timed) cudaEventRecord(c->evs[c->ev_used], c->stream);
+  switch (c->L.m) {
+    case 1: launch_stage_m<1>(c, A); break;
+    case 2: launch_stage_m<2>(c, A); break;
+    case 3: launch_stage_m<3>(c, A); break;
+    case 4: launch_stage_m<4>(c, A); break;
+    default: launch_stage_m<5>(c, A); break;
+  }
+  c->launches++;
+  if (timed) {
+    cudaEventRecord(c->evs[c->ev_used + 1], c->stream);
+    c->ev_used += 2;
+  }
+  CUDA_TRY(c, cudaGetLastError());
+  return DG_OK;
+}
+
+template <typename F1, typename F2, typename F3, typename F4, typename F5>
+void dispatch_m(int m, F1 f1, F2 f2, F3 f3, F4 f4, F5 f5) {
+  switch (m) { case 1: f1(); break; case 2: f2(); break; case 3: f3(); break; case 4: f4(); break; default: f5(); }
+}
+
+int to_nodal(dg_ctx* c, const double* U, double* Q) {
+  dim3 grid(c->L.nbx, c->p.ny);
+  const int nx = c->p.nx, nbx = c->L.nbx;
+  cudaStream_t s = c->stream;
+  const ConvTables& CT = c->CT;
+  dispatch_m(c->L.m,
+             [&] { modal_to_nodal_kernel<1><<<grid, 32, 0, s>>>(U, Q, nx, nbx, CT); },
+             [&] { modal_to_nodal_kernel<2><<<grid, 32, 0, s>>>(U, Q, nx, nbx, CT); },
+             [&] { modal_to_nodal_kernel<3><<<grid, 32, 0, s>>>(U, Q, nx, nbx, CT); },
+             [&] { modal_to_nodal_kernel<4><<<grid, 32, 0, s>>>(U, Q, nx, nbx, CT); },
+             [&] { modal_to_nodal_kernel<5><<<grid, 32, 0, s>>>(U, Q, nx, nbx, CT); });
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  return DG_OK;
+}
+
+int to_modal(dg_ctx* c, const double* Q, double* U) {
+  dim3 grid(c->L.nbx, c->p.ny);
+  const int nx = c->p.nx, nbx = c->L.nbx;
+  cudaStream_t s = c->stream;
+  const ConvTables& CT = c->CT;
+  dispatch_m(c->L.m,
+             [&] { nodal_to_modal_kernel<1><<<grid, 32, 0, s>>>(Q, U, nx, nbx, CT); },
+             [&] { nodal_to_modal_kernel<2><<<grid, 32, 0, s>>>(Q, U, nx, nbx, CT); },
+             [&] { nodal_to_modal_kernel<3><<<grid, 32, 0, s>>>(Q, U, nx, nbx, CT); },
+             [&] { nodal_to_modal_kernel<4><<<grid, 32, 0, s>>>(Q, U, nx, nbx, CT); },
+             [&] { nodal_to_modal_kernel<5><<<grid, 32, 0, s>>>(Q, U, nx, nbx, CT); });
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  return DG_OK;
+}
+
+int finish_set_state(dg_ctx* c) {
+  // q(cur) holds the new nodal state: snapshot it and its boundary traces where needed
+  if (c->L.need_q0)
+    CUDA_TRY(c, cudaMemcpyAsync(c->q0(), c->q(c->cur), c->L.state_doubles * sizeof(double),
+                                cudaMemcpyDeviceToDevice, c->stream));
+  if (c->L.need_btr) {
+    const int n = std::max(c->p.ny * 4 * c->L.m, c->L.nbx * 4 * c->L.m * 32);
+    const int blocks = (n + 127) / 128;
+    cudaStream_t s = c->stream;
+    dispatch_m(c->L.m,
+               [&] { boundary_trace_kernel<1><<<blocks, 128, 0, s>>>(c->q0(), c->btrW(), c->btrE(), c->btrS(), c->btrN(), c->g, c->T); },
+               [&] { boundary_trace_kernel<2><<<blocks, 128, 0, s>>>(c->q0(), c->btrW(), c->btrE(), c->btrS(), c->btrN(), c->g, c->T); },
+               [&] { boundary_trace_kernel<3><<<blocks, 128, 0, s>>>(c->q0(), c->btrW(), c->btrE(), c->btrS(), c->btrN(), c->g, c->T); },
+               [&] { boundary_trace_kernel<4><<<blocks, 128, 0, s>>>(c->q0(), c->btrW(), c->btrE(), c->btrS(), c->btrN(), c->g, c->T); },
+               [&] { boundary_trace_kernel<5><<<blocks, 128, 0, s>>>(c->q0(), c->btrW(), c->btrE(), c->btrS(), c->btrN(), c->g, c->T); });
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+  }
+  c->has_state = true;
+  c->wmax_valid = false;
+  c->t = c->p.t0;
+  return DG_OK;
+}
+
+int launch_damp(dg_ctx* c, double* Q, double dt) {
+  dim3 grid(c->L.nbx, (c->p.ny + 3) / 4);
+  const double r0 = c->p.damp_r0, inv_w = 1.0 / (c->p.damp_r1 - c->p.damp_r0);
+  const double tau0 = 2.0 * 3.14159265358979323846 * std::sqrt(r0 * r0 * r0 / c->p.gm_star);
+  cudaStream_t s = c->stream;
+  const double* Q0 = c->q0();
+  const Geom g = c->g;
+  dispatch_m(c->L.m,
+             [&] { damp_kernel<1><<<grid, 128, 0, s>>>(Q, Q0, g, dt, r0, inv_w, tau0); },
+             [&] { damp_kernel<2><<<grid, 128, 0, s>>>(Q, Q0, g, dt, r0, inv_w, tau0); },
+             [&] { damp_kernel<3><<<grid, 128, 0, s>>>(Q, Q0, g, dt, r0, inv_w, tau0); },
+             [&] { damp_kernel<4><<<grid, 128, 0, s>>>(Q, Q0, g, dt, r0, inv_w, tau0); },
+             [&] { damp_kernel<5><<<grid, 128, 0, s>>>(Q, Q0, g, dt, r0, inv_w, tau0); });
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  return DG_OK;
+}
+
+int do_step(dg_ctx* c, double dt, double* stages) {
+  if (!c) return DG_EINVAL;
+  if (!c->has_state) return fail(c, DG_ESTATE, "dg_step: state not set");
+  if (!(dt >= 0.0) || !std::isfinite(dt)) return fail(c, DG_EINVAL, "dg_step: bad dt");
+  const int A = c->cur, B = (c->cur + 1) % 3, Cc = (c->cur + 2) % 3;
+  const size_t n = (size_t)c->p.ny * c->p.nx * 4 * c->L.m * c->L.m;
+  const bool damp = c->p.damp_r0 > 0.0;
+  int last = (damp ? F_DAMP : 0) | (c->fused_cfl ? F_CFL : 0);
+  if (stages) last = 0;      // debug stages are "before damping": damping runs as its own pass below
+  int e;
+  if (c->fused_cfl && !stages)
+    CUDA_TRY(c, cudaMemsetAsync(c->wmax(), 0, sizeof(unsigned long long), c->stream));
+  // SSP-RK in Shu-Osher form, stage times c = (0,1) / (0,1,1/2)
+  if ((e = launch_stage(c, c->q(A), c->q(A), c->q(B), 0.0, 1.0, dt, c->t, F_NO_UN))) return e;
+  if (stages && (e = to_modal(c, c->q(B), stages))) return e;
+  if (c->p.rk == 2) {
+    if ((e = launch_stage(c, c->q(B), c->q(A), c->q(Cc), 0.5, 0.5, dt, c->t + dt, last))) return e;
+    if (stages && (e = to_modal(c, c->q(Cc), stages + n))) return e;
+    c->cur = Cc;
+  } else {
+    if ((e = launch_stage(c, c->q(B), c->q(A), c->q(Cc), 0.75, 0.25, dt, c->t + dt, 0))) return e;
+    if (stages && (e = to_modal(c, c->q(Cc), stages + n))) return e;
+    if ((e = launch_stage(c, c->q(Cc), c->q(A), c->q(B), 1.0 / 3.0, 2.0 / 3.0, dt, c->t + 0.5 * dt, last))) return e;
+    if (stages && (e = to_modal(c, c->q(B), stages + 2 * n))) return e;
+    c->cur = B;
+  }
+  c->wmax_valid = c->fused_cfl && !stages;
+  if (stages && damp) {   // debug path: stages are "before damping", so relax in a separate pass
+    if ((e = launch_damp(c, c->q(c->cur), dt))) return e;
+  }
+  c->t += dt;
+  return DG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t dg_workspace_bytes(const dg_params* p) {
+  if (!valid_params(p)) return 0;
+  return make_layout(p).total;
+}
+
+int dg_init(const dg_params* p, void* workspace, size_t ws_bytes, void* cuda_stream, dg_ctx** out) {
+  if (!out) return DG_EINVAL;
+  *out = nullptr;
+  if (!valid_params(p) || !workspace) return DG_EINVAL;
+  if (reinterpret_cast<uintptr_t>(workspace) % ALIGN) return DG_EINVAL;
+  Layout L = make_layout(p);
+  if (ws_bytes < L.total) return DG_ENOSPC;
+  dg_ctx* c = new (std::nothrow) dg_ctx();
+  if (!c) return DG_EINVAL;
+  c->p = *p;
+  c->L = L;
+  c->stream = static_cast<cudaStream_t>(cuda_stream);
+  c->ws = static_cast<char*>(workspace);
+  c->cur = 0;
+  c->has_state = false;
+  c->wmax_valid = false;
+  c->t = p->t0;
+  c->rows_per_cta = 16;
+  c->fused_cfl = 1;
+  c->launches = 0;
+  c->timing = false;
+  c->ev_used = 0;
+  build_host_tables(p->order, &c->H);
+  Geom& g = c->g;
+  g.x0 = p->x0; g.y0 = p->y0;
+  g.dx = (p->x1 - p->x0) / p->nx; g.dy = (p->y1 - p->y0) / p->ny;
+  g.hdx = 0.5 * g.dx; g.hdy = 0.5 * g.dy;
+  g.inv_dx = 1.0 / g.dx; g.inv_dy = 1.0 / g.dy;
+  g.nx = p->nx; g.ny = p->ny; g.nbx = L.nbx; g.bc = p->bc;
+  std::memset(&c->T, 0, sizeof c->T);
+  std::memset(&c->CT, 0, sizeof c->CT);
+  for (int q = 0; q < p->order; ++q) {
+    c->T.xi[q] = c->H.xi[q]; c->T.w[q] = c->H.w[q];
+    c->T.lxp[q] = c->H.lp[q] / g.dx; c->T.lxm[q] = c->H.lm[q] / g.dx;
+    c->T.lyp[q] = c->H.lp[q] / g.dy; c->T.lym[q] = c->H.lm[q] / g.dy;
+    c->T.Ip[q] = c->H.Ip[q]; c->T.Im[q] = c->H.Im[q];
+    for (int k = 0; k < p->order; ++k) {
+      c->T.Dx[q][k] = c->H.Dh[q][k] / g.dx;
+      c->T.Dy[q][k] = c->H.Dh[q][k] / g.dy;
+      c->CT.B[q][k] = c->H.B[q][k];
+      c->CT.P[q][k] = c->H.P[q][k];
+    }
+  }
+  *out = c;
+  return DG_OK;
+}
+
+int dg_set_state(dg_ctx* c, const double* U) {
+  if (!c || !U) return c ? fail(c, DG_EINVAL, "dg_set_state: null") : DG_EINVAL;
+  c->cur = 0;
+  int e = to_nodal(c, U, c->q(0));
+  if (e) return e;
+  return finish_set_state(c);
+}
+
+int dg_set_state_host(dg_ctx* c, const double* U) {
+  if (!c || !U) return c ? fail(c, DG_EINVAL, "dg_set_state_host: null") : DG_EINVAL;
+  const size_t bytes = (size_t)c->p.ny * c->p.nx * 4 * c->L.m * c->L.m * sizeof(double);
+  c->cur = 0;
+  double* staging = c->q(2);            // modal bytes <= one state buffer
+  CUDA_TRY(c, cudaMemcpyAsync(staging, U, bytes, cudaMemcpyHostToDevice, c->stream));
+  int e = to_nodal(c, staging, c->q(0));
+  if (e) return e;
+  return finish_set_state(c);
+}
+
+int dg_get_state(dg_ctx* c, double* U) {
+  if (!c || !U) return c ? fail(c, DG_EINVAL, "dg_get_state: null") : DG_EINVAL;
+  if (!c->has_state) return fail(c, DG_ESTATE, "dg_get_state: state not set");
+  return to_modal(c, c->q(c->cur), U);
+}
+
+int dg_get_state_host(dg_ctx* c, double* U) {
+  if (!c || !U) return c ? fail(c, DG_EINVAL, "dg_get_state_host: null") : DG_EINVAL;
+  if (!c->has_state) return fail(c, DG_ESTATE, "dg_get_state_host: state not set");
+  const size_t bytes = (size_t)c->p.ny * c->p.nx * 4 * c->L.m * c->L.m * sizeof(double);
+  double* staging = c->q((c->cur + 1) % 3);
+  int e = to_modal(c, c->q(c->cur), staging);
+  if (e) return e;
+  CUDA_TRY(c, cudaMemcpyAsync(U, staging, bytes, cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return DG_OK;
+}
+
+int dg_rhs(dg_ctx* c, double t, double* Lout) {
+  if (!c || !Lout) return c ? fail(c, DG_EINVAL, "dg_rhs: null") : DG_EINVAL;
+  if (!c->has_state) return fail(c, DG_ESTATE, "dg_rhs: state not set");
+  double* scratch = c->q((c->cur + 1) % 3);
+  int e = launch_stage(c, c->q(c->cur), c->q(c->cur), scratch, 0.0, 1.0, 0.0, t, F_RHS_ONLY | F_NO_UN);
+  if (e) return e;
+  return to_modal(c, scratch, Lout);
+}
+
+int dg_cfl_dt(dg_ctx* c, double cfl, double* dt) {
+  if (!c || !dt) return c ? fail(c, DG_EINVAL, "dg_cfl_dt: null") : DG_EINVAL;
+  if (!c->has_state) return fail(c, DG_ESTATE, "dg_cfl_dt: state not set");
+  if (!c->wmax_valid) {
+    CUDA_TRY(c, cudaMemsetAsync(c->wmax(), 0, sizeof(unsigned long long), c->stream));
+    dim3 grid(c->L.nbx, (c->p.ny + 3) / 4);
+    const Phys ph = make_phys(c, c->t);
+    cudaStream_t s = c->stream;
+    const double* Q = c->q(c->cur);
+    const int eos = c->p.eos;
+    auto go = [&](auto tag) {
+      constexpr int M = decltype(tag)::value;
+      if (eos == 0) cfl_kernel<M, 0><<<grid, 128, 0, s>>>(Q, c->wmax(), c->g, ph, c->T);
+      else          cfl_kernel<M, 1><<<grid, 128, 0, s>>>(Q, c->wmax(), c->g, ph, c->T);
+    };
+    dispatch_m(c->L.m, [&] { go(std::integral_constant<int, 1>{}); }, [&] { go(std::integral_constant<int, 2>{}); },
+               [&] { go(std::integral_constant<int, 3>{}); }, [&] { go(std::integral_constant<int, 4>{}); },
+               [&] { go(std::integral_constant<int, 5>{}); });
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+    c->wmax_valid = true;
+  }
+  double worst = 0.0;
+  CUDA_TRY(c, cudaMemcpyAsync(&worst, c->wmax(), sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  *dt = cfl / (2.0 * (c->L.m - 1) + 1.0) / worst;
+  return DG_OK;
+}
+
+int dg_step(dg_ctx* c, double dt) { return do_step(c, dt, nullptr); }
+int dg_step_debug(dg_ctx* c, double dt, double* stages) {
+  if (!stages) return c ? fail(c, DG_EINVAL, "dg_step_debug: null") : DG_EINVAL;
+  return do_step(c, dt, stages);
+}
+
+int dg_run_host(dg_ctx* c, const double* U_in, int nsteps, double cfl, double* U_out) {
+  if (!c || !U_in || !U_out || nsteps < 0) return c ? fail(c, DG_EINVAL, "dg_run_host: bad argument") : DG_EINVAL;
+  int e = dg_set_state_host(c, U_in);
+  for (int k = 0; !e && k < nsteps; ++k) {
+    double dt;
+    e = dg_cfl_dt(c, cfl, &dt);
+    if (!e) e = dg_step(c, dt);
+  }
+  if (!e) e = dg_get_state_host(c, U_out);
+  return e;
+}
+
+double dg_time(const dg_ctx* c) { return c ? c->t : 0.0; }
+int dg_set_time(dg_ctx* c, double t) {
+  if (!c) return DG_EINVAL;
+  c->t = t;
+  return DG_OK;
+}
+long long dg_launch_count(const dg_ctx* c) { return c ? c->launches : 0; }
+
+int dg_set_tuning(dg_ctx* c, int key, int value) {
+  if (!c) return DG_EINVAL;
+  switch (key) {
+    case DG_TUNE_ROWS_PER_CTA:
+      if (value < 1) return fail(c, DG_EINVAL, "rows per CTA must be >= 1");
+      c->rows_per_cta = value;
+      return DG_OK;
+    case DG_TUNE_FUSED_CFL:
+      c->fused_cfl = value ? 1 : 0;
+      c->wmax_valid = false;
+      return DG_OK;
+    default:
+      return fail(c, DG_EINVAL, "unknown tuning key");
+  }
+}
+
+int dg_stage_timing(dg_ctx* c, int enable) {
+  if (!c) return DG_EINVAL;
+  const size_t want = 2 * 4096;       // up to 4096 stage launches per measurement window
+  while (enable && c->evs.size() < want) {
+    cudaEvent_t e;
+    CUDA_TRY(c, cudaEventCreate(&e));
+    c->evs.push_back(e);
+  }
+  c->timing = enable != 0;
+  c->ev_used = 0;
+  return DG_OK;
+}
+
+int dg_stage_time_ms(dg_ctx* c, double* mean_ms, long long* launches) {
+  if (!c || !mean_ms || !launches) return DG_EINVAL;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  double sum = 0.0;
+  for (size_t k = 0; k + 1 < c->ev_used; k += 2) {
+    float ms = 0.f;
+    CUDA_TRY(c, cudaEventElapsedTime(&ms, c->evs[k], c->evs[k + 1]));
+    sum += ms;
+  }
+  *launches = (long long)(c->ev_used / 2);
+  *mean_ms = c->ev_used ? sum / (double)(c->ev_used / 2) : 0.0;
+  return DG_OK;
+}
+
+int dg_probe_fp64_peak(dg_ctx* c, double* tflops) {
+  if (!c || !tflops) return DG_EINVAL;
+  int dev = 0, sms = 0;
+  CUDA_TRY(c, cudaGetDevice(&dev));
+  CUDA_TRY(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  cudaEvent_t a, b;
+  CUDA_TRY(c, cudaEventCreate(&a));
+  CUDA_TRY(c, cudaEventCreate(&b));
+  const int iters = 1 << 15, blocks = sms * 8, threads = 256;
+  double* out = reinterpret_cast<double*>(c->ws + c->L.off_scalars + 64);
+  double best = 0.0;
+  for (int rep = 0; rep < 5; ++rep) {
+    cudaEventRecord(a, c->stream);
+    dfma_probe_kernel<<<blocks, threads, 0, c->stream>>>(out, iters, 1.0 + rep);
+    cudaEventRecord(b, c->stream);
+    CUDA_TRY(c, cudaEventSynchronize(b));
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    const double fl = 2.0 * 8.0 * (double)iters * blocks * threads;
+    if (rep > 0 && ms > 0.f) best = std::max(best, fl / (ms * 1e-3) / 1e12);
+    c->launches++;
+  }
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  *tflops = best;
+  return DG_OK;
+}
+
+const char* dg_last_error(const dg_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+void dg_destroy(dg_ctx* c) {
+  if (!c) return;
+  for (cudaEvent_t e : c->evs) cudaEventDestroy(e);
+  delete c;
+}
+
+}  // extern "C"
