@@ -126,11 +126,21 @@ Phys make_phys(const dg_ctx* c, double t) {
   return ph;
 }
 
+template <int M, int EOS>
+void launch_stage_me(dg_ctx* c, const StageArgs& A) {
+  static bool attr_set = false;      // dynamic shared memory above 48 KB must be opted in once
+  constexpr size_t smem = stage_smem_bytes<M>();
+  if (!attr_set) {
+    cudaFuncSetAttribute(stage_kernel<M, EOS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr_set = true;
+  }
+  dim3 grid(c->L.nbx, (c->p.ny + A.rows - 1) / A.rows), block(M * 32);
+  stage_kernel<M, EOS><<<grid, block, smem, c->stream>>>(A);
+}
 template <int M>
 int launch_stage_m(dg_ctx* c, const StageArgs& A) {
-  dim3 grid(c->L.nbx, (c->p.ny + A.rows - 1) / A.rows), block(M * 32);
-  if (c->p.eos == 0) stage_kernel<M, 0><<<grid, block, 0, c->stream>>>(A);
-  else               stage_kernel<M, 1><<<grid, block, 0, c->stream>>>(A);
+  if (c->p.eos == 0) launch_stage_me<M, 0>(c, A);
+  else               launch_stage_me<M, 1>(c, A);
   return 0;
 }
 

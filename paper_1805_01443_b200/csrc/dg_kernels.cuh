@@ -70,17 +70,40 @@ struct StageArgs {
 };
 
 // ---------------------------------------------------------------------------------------------
+// fp64 special functions without slow paths: MUFU seed (~20 bits) + 2 Newton steps (measured max
+// relative error 1.1e-16 / 1.4e-16 on B200).  Arguments are positive and normal here.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double rcp_fast(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
+}
+__device__ __forceinline__ double rsqrt_fast(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-(x * y), y, 1.0);
+  y = fma(0.5 * y, e, y);
+  e = fma(-(x * y), y, 1.0);
+  return fma(0.5 * y, e, y);
+}
+__device__ __forceinline__ double sqrt_fast(double x) { return x * rsqrt_fast(x); }
+
+// ---------------------------------------------------------------------------------------------
 // Point-wise physics (rows a2, a3, a6)
 // ---------------------------------------------------------------------------------------------
 // Euler flux in direction DIR of the conservative state u (Eq.(1)) with the closure
-// Eq.(2) PAPER.md:45-49 (EOS 0) or p = c_s^2 rho (EOS 1).  LAM: also |v_n| + c.
+// Eq.(2) PAPER.md:45-49 (EOS 0) or p = c_s^2 rho (EOS 1: cs2 and c = sqrt(cs2) are passed in).
+// LAM: also the signal speed |v_n| + c.
 template <int EOS, int DIR, bool LAM>
-__device__ __forceinline__ void euler_flux(const Phys& ph, const double (&u)[4], double cs2,
+__device__ __forceinline__ void euler_flux(const Phys& ph, const double (&u)[4], double cs2, double ciso,
                                            double (&F)[4], double& lam) {
-  const double rinv = 1.0 / u[0];
+  const double rinv = rcp_fast(u[0]);
   const double vx = u[1] * rinv, vy = u[2] * rinv;
   double pr;
-  if (EOS == 0) pr = ph.gm1 * (u[3] - 0.5 * (u[1] * vx + u[2] * vy));
+  if (EOS == 0) pr = ph.gm1 * (u[3] - 0.5 * fma(u[1], vx, u[2] * vy));
   else          pr = cs2 * u[0];
   const double vn = DIR == 0 ? vx : vy;
   F[0] = u[1 + DIR];
@@ -88,50 +111,44 @@ __device__ __forceinline__ void euler_flux(const Phys& ph, const double (&u)[4],
   F[2] = DIR == 1 ? fma(u[2], vn, pr) : u[2] * vn;
   F[3] = (u[3] + pr) * vn;
   if (LAM) {
-    const double c = EOS == 0 ? sqrt(ph.gamma * pr * rinv) : sqrt(cs2);
+    const double c = EOS == 0 ? sqrt_fast(ph.gamma * pr * rinv) : ciso;
     lam = fabs(vn) + c;
   }
 }
 
 // Local Lax-Friedrichs flux from the two sides' states, fluxes and speeds.
-// Always called with (left, right) in the same order by both cells sharing the face, on bitwise
-// identical operands, so the interface flux is single valued to the last bit.
+// Each interior face is evaluated exactly once (by the cell on its left / below) and handed to the
+// other cell, so the interface flux is single valued to the last bit.
 __device__ __forceinline__ void llf(const double (&UL)[4], const double (&FL)[4], double lamL,
                                     const double (&UR)[4], const double (&FR)[4], double lamR,
                                     double (&H)[4]) {
   const double hl = 0.5 * fmax(lamL, lamR);
 #pragma unroll
-  for (int v = 0; v < 4; ++v) H[v] = 0.5 * (FL[v] + FR[v]) - hl * (UR[v] - UL[v]);
-}
-
-template <int EOS>
-__device__ __forceinline__ double cs2_iso(const Phys& ph, double x, double y) {
-  return EOS == 1 ? ph.h2gm * rsqrt(fma(x, x, fma(y, y, ph.eps2s))) : 0.0;
+  for (int v = 0; v < 4; ++v) H[v] = fma(-hl, UR[v] - UL[v], 0.5 * (FL[v] + FR[v]));
 }
 
 // ---------------------------------------------------------------------------------------------
-// Traces of a neighbouring cell read straight from global memory (block edges, halo rows)
+// Traces of a cell (node stride `s` doubles: 32 inside a tile, 1 inside the edge buffer)
 // ---------------------------------------------------------------------------------------------
-// cell points at element [v=0][r=0][q=0] of the cell (block base + lane); node stride is 32.
 template <int M>
-__device__ __forceinline__ void line_trace(const double* __restrict__ cell, int r,
+__device__ __forceinline__ void line_trace(const double* cell, int stride, int r,
                                            const double (&I)[MAXM], double (&out)[4]) {
 #pragma unroll
   for (int v = 0; v < 4; ++v) {
     double s = 0.0;
 #pragma unroll
-    for (int q = 0; q < M; ++q) s = fma(I[q], __ldg(cell + ((v * M + r) * M + q) * 32), s);
+    for (int q = 0; q < M; ++q) s = fma(I[q], cell[((v * M + r) * M + q) * stride], s);
     out[v] = s;
   }
 }
 template <int M>
-__device__ __forceinline__ void column_trace(const double* __restrict__ cell, int q,
+__device__ __forceinline__ void column_trace(const double* cell, int stride, int q,
                                              const double (&I)[MAXM], double (&out)[4]) {
 #pragma unroll
   for (int v = 0; v < 4; ++v) {
     double s = 0.0;
 #pragma unroll
-    for (int r = 0; r < M; ++r) s = fma(I[r], __ldg(cell + ((v * M + r) * M + q) * 32), s);
+    for (int r = 0; r < M; ++r) s = fma(I[r], cell[((v * M + r) * M + q) * stride], s);
     out[v] = s;
   }
 }
@@ -140,59 +157,218 @@ __device__ __forceinline__ double shfl_up1(double x) { return __shfl_up_sync(FUL
 __device__ __forceinline__ double shfl_dn1(double x) { return __shfl_down_sync(FULL, x, 1); }
 
 // ---------------------------------------------------------------------------------------------
-// The fused RK-stage kernel (rows a2..a9, a11, a12 of SURVEY.md 8(a); a1/a4's basis change is
-// algebraically folded into the tables, see dg_tables.h)
+// TMA (bulk async copy) + mbarrier helpers: one contiguous 32-cell tile per copy
 // ---------------------------------------------------------------------------------------------
-template <int M, int EOS>
-__global__ void __launch_bounds__(M * 32)
-stage_kernel(const __grid_constant__ StageArgs A) {
-  __shared__ double sN[4 * M * M * 32];          // x-direction part of N, [v][r][q][lane]
-  __shared__ double sAvg[(M > 1 ? M : 1) * 4 * 32];
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
 
-  const int lane = threadIdx.x & 31;
-  const int w = threadIdx.x >> 5;                // line index (X phase) / column index (Y phase)
+// ---------------------------------------------------------------------------------------------
+// The fused RK-stage kernel (rows a2..a12 of SURVEY.md 8(a); a1/a4's basis change is folded into
+// the tables, see dg_tables.h).
+//
+// Shared memory of one thread block (M warps, one 32-cell column block, `rows` rows):
+//   tiles[3]  ring of u^(s-1) tiles (rows j-1 | j | j+1 | j+2 rotating), each one contiguous
+//             4 M^2 x 32 doubles in HBM -> filled by ONE cp.async.bulk (TMA) each, mbarrier-tracked;
+//             the copy for row j+2 is in flight while row j is computed
+//   sN        x-direction part of N for the row in flight ([v][r][q][lane]; transposes ownership
+//             from eta-lines to xi-columns)
+//   sRi       1/sqrt(x^2+y^2+eps^2) at the row's volume nodes (shared by c_s^2 and the star gravity)
+//   sEdge[2]  the two x-neighbour cells outside the block, prefetched one row ahead
+// ---------------------------------------------------------------------------------------------
+#ifndef DG_STAGE_MINB
+#define DG_STAGE_MINB 2
+#endif
+constexpr int NST = 3;
+
+template <int M>
+constexpr size_t stage_smem_bytes() {
+  // tiles + sN + sRi + sEdge + mbarriers
+  return ((size_t)(NST + 1) * 4 * M * M * 32 + (size_t)M * M * 32 + (size_t)4 * 4 * M * M) * sizeof(double) + 64;
+}
+
+template <int M, int EOS>
+__global__ void __launch_bounds__(M * 32, DG_STAGE_MINB)
+stage_kernel(const __grid_constant__ StageArgs A) {
+  constexpr int C = 4 * M * M;                   // doubles per cell
+  constexpr int BS = C * 32;                     // doubles per 32-cell tile
+  constexpr int NT = M * 32;
+  constexpr uint32_t TILE_BYTES = BS * sizeof(double);
+  extern __shared__ __align__(128) double smem[];
+  double* tiles = smem;
+  double* sN = tiles + NST * BS;
+  double* sRi = sN + BS;                         // [r][q][lane]
+  double* sEdge = sRi + M * M * 32;              // [slot][side][C]
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(sEdge + 4 * C);
+
+  const int tid = threadIdx.x;
+  const int lane = tid & 31;
+  const int w = tid >> 5;                        // eta-line (X phase) / xi-column (Y phase)
   const int ib = blockIdx.x;
   const int i = ib * 32 + lane;
   const Geom& g = A.g;
   const DevTables& T = A.T;
   const bool valid = i < g.nx;
+  const int last_lane = min(31, g.nx - 1 - ib * 32);
   const int j0 = blockIdx.y * A.rows;
   const int j1 = min(g.ny, j0 + A.rows);
-  constexpr int C = 4 * M * M;                   // doubles per cell
-  constexpr size_t BS = (size_t)C * 32;          // doubles per 32-cell block
   const size_t row_stride = (size_t)g.nbx * BS;
+  const bool grav = (A.flags & F_GRAV) != 0;
+  const bool need_ri = EOS == 1 || grav;
 
   const double xc = g.x0 + (i + 0.5) * g.dx;
   const double xW = g.x0 + i * g.dx, xE = g.x0 + (i + 1) * g.dx;
   const double xq_col = xc + g.hdx * T.xi[w];    // x of this thread's column (Y phase)
 
-  // ---- data of the row below (its N-face trace, flux, speed) for the Y phase, column q = w ----
-  double bU[4], bG[4], bLam;
+  // x-neighbour cells outside this block: (cell index, or -1 when there is none)
+  const int iLn = ib > 0 ? ib * 32 - 1 : (g.bc == 0 ? g.nx - 1 : -1);
+  const int iRn = ib * 32 + 32 < g.nx ? ib * 32 + 32 : (g.bc == 0 ? 0 : -1);
+  const double* edgeL = iLn >= 0 ? A.qprev + (size_t)(iLn >> 5) * BS + (iLn & 31) : nullptr;
+  const double* edgeR = iRn >= 0 ? A.qprev + (size_t)(iRn >> 5) * BS + (iRn & 31) : nullptr;
+  constexpr int NE = (2 * C + NT - 1) / NT;      // edge elements per thread
+  auto edge_load = [&](int jj, double (&e)[NE]) {
+#pragma unroll
+    for (int k = 0; k < NE; ++k) {
+      const int idx = tid + k * NT;
+      e[k] = 0.0;
+      if (idx < 2 * C) {
+        const double* src = idx < C ? edgeL : edgeR;
+        const int el = idx < C ? idx : idx - C;
+        if (src) e[k] = __ldg(src + (size_t)jj * row_stride + el * 32);
+      }
+    }
+  };
+  auto edge_store = [&](int slot, const double (&e)[NE]) {
+#pragma unroll
+    for (int k = 0; k < NE; ++k) {
+      const int idx = tid + k * NT;
+      if (idx < 2 * C) sEdge[slot * 2 * C + idx] = e[k];
+    }
+  };
+
+  // tile t holds row j0-1+t (wrapped for periodic domains; absent outside a non-periodic domain)
+  auto tile_row = [&](int t) -> int {
+    const int jj = j0 - 1 + t;
+    if (jj < 0) return g.bc == 0 ? g.ny - 1 : -1;
+    if (jj >= g.ny) return g.bc == 0 ? 0 : -1;
+    return jj;
+  };
+  auto tile_issue = [&](int t) {
+    const int jr = tile_row(t);
+    if (tid == 0 && jr >= 0) {
+      uint64_t* bar = mbar + t % NST;
+      mbar_expect_tx(bar, TILE_BYTES);
+      bulk_g2s(tiles + (t % NST) * BS, A.qprev + jr * row_stride + (size_t)ib * BS, TILE_BYTES, bar);
+    }
+  };
+  // k-th copy into a slot completes mbarrier phase k; tile 0 is the only one that can be absent
+  // and still be followed by later copies into its slot (non-periodic bottom row)
+  const int skip0 = tile_row(0) < 0 ? 1 : 0;
+  auto tile_wait = [&](int t) {
+    if (tile_row(t) >= 0) mbar_wait(mbar + t % NST, (uint32_t)((t / NST - (t % NST == 0 ? skip0 : 0)) & 1));
+  };
+
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < NST; ++s) mbar_init(mbar + s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  tile_issue(0);
+  tile_issue(1);
+  tile_issue(2);
   {
+    double e[NE];
+    edge_load(j0, e);
+    edge_store(j0 & 1, e);
+  }
+
+  // numerical flux through the south face of the row about to be processed, column q = w
+  double HS[4];
+  bool have_HS = false;
+  double bU[4], bG[4], bLam = 0.0;               // north-face data of the row below (first row only)
+  bool have_below = false;
+  {
+    tile_wait(0);
     const double yS = g.y0 + j0 * g.dy;
-    const double cs2 = cs2_iso<EOS>(A.ph, xq_col, yS);
-    bool have = true;
-    if (j0 > 0 || g.bc == 0) {
-      const int jj = j0 > 0 ? j0 - 1 : g.ny - 1;
-      column_trace<M>(A.qprev + jj * row_stride + ib * BS + lane, w, T.Ip, bU);
+    double cs2 = 0.0, ciso = 0.0;
+    if (EOS == 1) {
+      cs2 = A.ph.h2gm * rsqrt_fast(fma(xq_col, xq_col, fma(yS, yS, A.ph.eps2s)));
+      ciso = sqrt_fast(cs2);
+    }
+    if (tile_row(0) >= 0) {
+      column_trace<M>(tiles + lane, 32, w, T.Ip, bU);
+      have_below = true;
     } else if (g.bc == 2) {
 #pragma unroll
       for (int v = 0; v < 4; ++v) bU[v] = __ldg(A.btrS + ((size_t)(ib * 4 + v) * M + w) * 32 + lane);
-    } else {
-      have = false;                              // transmissive: filled from the own trace below
+      have_below = true;
     }
-    if (have) euler_flux<EOS, 1, true>(A.ph, bU, cs2, bG, bLam);
-    else { bLam = -1.0; }
+    if (have_below) euler_flux<EOS, 1, true>(A.ph, bU, cs2, ciso, bG, bLam);
   }
+  __syncthreads();                               // tile 0's slot may be refilled; sEdge[j0&1] visible
 
   for (int j = j0; j < j1; ++j) {
-    const double* __restrict__ qb = A.qprev + j * row_stride + ib * BS + lane;
+    const int t = j - j0 + 1;                    // tile index of row j
+    if (j + 1 < j1) tile_issue(t + 2);           // row j+2 -> the slot row j-1 has just left
+    const double* tu = tiles + (t % NST) * BS + lane;
     const double yc = g.y0 + (j + 0.5) * g.dy;
+    double enext[NE];
+    const bool more = j + 1 < j1;
+    if (more) edge_load(j + 1, enext);
 
+    // fused CFL wave speed of the row finished in the previous iteration (row a10).
+    // Partial cell averages were parked in sN[v][r=0][q][lane], which only this warp rewrites.
+    if ((A.flags & F_CFL) && w == 0 && j > j0) {
+      double avg[4];
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        double s = 0.0;
+#pragma unroll
+        for (int qq = 0; qq < M; ++qq) s += sN[((v * M + 0) * M + qq) * 32 + lane];
+        avg[v] = s;
+      }
+      double sp = 0.0;
+      if (valid) {
+        const double ycp = g.y0 + (j - 0.5) * g.dy;
+        const double rinv = 1.0 / avg[0];
+        const double vx = avg[1] * rinv, vy = avg[2] * rinv;
+        double c;
+        if (EOS == 0) c = sqrt(A.ph.gamma * A.ph.gm1 * (avg[3] - 0.5 * (avg[1] * vx + avg[2] * vy)) * rinv);
+        else          c = sqrt(A.ph.h2gm * rsqrt(fma(xc, xc, fma(ycp, ycp, A.ph.eps2s))));
+        sp = (fabs(vx) + c) * g.inv_dx + (fabs(vy) + c) * g.inv_dy;
+        if (!(sp >= 0.0)) sp = __longlong_as_double(0x7ff0000000000000LL);   // NaN -> +inf
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) sp = fmax(sp, __shfl_xor_sync(FULL, sp, o));
+      if (lane == 0) atomicMax(A.wmax, (unsigned long long)__double_as_longlong(sp));
+    }
+
+    tile_wait(t);
     // =========================== X phase: eta-line r = w ===========================
     {
       const int r = w;
       const double yr = yc + g.hdy * T.xi[r];
+      const double y2e = fma(yr, yr, A.ph.eps2s);
       double acc[4][M];
 #pragma unroll
       for (int v = 0; v < 4; ++v)
@@ -203,49 +379,48 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       for (int q = 0; q < M; ++q) {
         double u[4];
 #pragma unroll
-        for (int v = 0; v < 4; ++v) u[v] = __ldg(qb + ((v * M + r) * M + q) * 32);
+        for (int v = 0; v < 4; ++v) u[v] = tu[((v * M + r) * M + q) * 32];
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
           UW[v] = fma(T.Im[q], u[v], UW[v]);
           UE[v] = fma(T.Ip[q], u[v], UE[v]);
         }
-        const double xq = xc + g.hdx * T.xi[q];
+        double cs2 = 0.0;
+        if (need_ri) {
+          const double xq = xc + g.hdx * T.xi[q];
+          const double ri = rsqrt_fast(fma(xq, xq, y2e));
+          sRi[(r * M + q) * 32 + lane] = ri;
+          if (EOS == 1) cs2 = A.ph.h2gm * ri;
+        }
         double F[4], dummy;
-        euler_flux<EOS, 0, false>(A.ph, u, cs2_iso<EOS>(A.ph, xq, yr), F, dummy);
+        euler_flux<EOS, 0, false>(A.ph, u, cs2, 0.0, F, dummy);
 #pragma unroll
         for (int v = 0; v < 4; ++v)
 #pragma unroll
           for (int qq = 0; qq < M; ++qq) acc[v][qq] = fma(T.Dx[qq][q], F[v], acc[v][qq]);
       }
-      // own face data, then the neighbours' by shuffle (left cell's E face, right cell's W face)
-      double FWo[4], FEo[4], lamWo, lamEo;
-      euler_flux<EOS, 0, true>(A.ph, UW, cs2_iso<EOS>(A.ph, xW, yr), FWo, lamWo);
-      euler_flux<EOS, 0, true>(A.ph, UE, cs2_iso<EOS>(A.ph, xE, yr), FEo, lamEo);
-      double UL[4], FL[4], lamL, UR[4], FR[4], lamR;
-#pragma unroll
-      for (int v = 0; v < 4; ++v) {
-        UL[v] = shfl_up1(UE[v]);  FL[v] = shfl_up1(FEo[v]);
-        UR[v] = shfl_dn1(UW[v]);  FR[v] = shfl_dn1(FWo[v]);
-      }
-      lamL = shfl_up1(lamEo);
-      lamR = shfl_dn1(lamWo);
-      if (valid && lane == 0) {                  // left neighbour lives in another block / outside
-        if (i > 0 || g.bc == 0) {
-          const int ii = i > 0 ? i - 1 : g.nx - 1;
-          line_trace<M>(A.qprev + j * row_stride + (size_t)(ii >> 5) * BS + (ii & 31), r, T.Ip, UL);
-        } else if (g.bc == 1) {
-#pragma unroll
-          for (int v = 0; v < 4; ++v) UL[v] = UW[v];
-        } else {
-#pragma unroll
-          for (int v = 0; v < 4; ++v) UL[v] = __ldg(A.btrW + ((size_t)j * 4 + v) * M + r);
+      // own W/E face states, fluxes, speeds; c_s at the E face is the right neighbour's W value
+      double cs2W = 0.0, cW = 0.0, cs2E = 0.0, cE = 0.0;
+      if (EOS == 1) {
+        cs2W = A.ph.h2gm * rsqrt_fast(fma(xW, xW, y2e));
+        cW = sqrt_fast(cs2W);
+        cs2E = shfl_dn1(cs2W);
+        cE = shfl_dn1(cW);
+        if (lane == 31) {
+          cs2E = A.ph.h2gm * rsqrt_fast(fma(xE, xE, y2e));
+          cE = sqrt_fast(cs2E);
         }
-        euler_flux<EOS, 0, true>(A.ph, UL, cs2_iso<EOS>(A.ph, xW, yr), FL, lamL);
       }
-      if (valid && (lane == 31 || i == g.nx - 1)) {
-        if (i < g.nx - 1 || g.bc == 0) {
-          const int ii = i < g.nx - 1 ? i + 1 : 0;
-          line_trace<M>(A.qprev + j * row_stride + (size_t)(ii >> 5) * BS + (ii & 31), r, T.Im, UR);
+      double FWo[4], FEo[4], lamWo, lamEo;
+      euler_flux<EOS, 0, true>(A.ph, UW, cs2W, cW, FWo, lamWo);
+      euler_flux<EOS, 0, true>(A.ph, UE, cs2E, cE, FEo, lamEo);
+      double UR[4], FR[4], lamR;
+#pragma unroll
+      for (int v = 0; v < 4; ++v) { UR[v] = shfl_dn1(UW[v]); FR[v] = shfl_dn1(FWo[v]); }
+      lamR = shfl_dn1(lamWo);
+      if (lane == last_lane) {                   // right neighbour is outside this block
+        if (edgeR) {
+          line_trace<M>(sEdge + (j & 1) * 2 * C + C, 1, r, T.Im, UR);
         } else if (g.bc == 1) {
 #pragma unroll
           for (int v = 0; v < 4; ++v) UR[v] = UE[v];
@@ -253,11 +428,26 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 #pragma unroll
           for (int v = 0; v < 4; ++v) UR[v] = __ldg(A.btrE + ((size_t)j * 4 + v) * M + r);
         }
-        euler_flux<EOS, 0, true>(A.ph, UR, cs2_iso<EOS>(A.ph, xE, yr), FR, lamR);
+        euler_flux<EOS, 0, true>(A.ph, UR, cs2E, cE, FR, lamR);
       }
-      double HW[4], HE[4];
-      llf(UL, FL, lamL, UW, FWo, lamWo, HW);
+      double HE[4], HW[4];
       llf(UE, FEo, lamEo, UR, FR, lamR, HE);
+#pragma unroll
+      for (int v = 0; v < 4; ++v) HW[v] = shfl_up1(HE[v]);
+      if (lane == 0) {                           // left neighbour is outside this block
+        double UL[4], FL[4], lamL;
+        if (edgeL) {
+          line_trace<M>(sEdge + (j & 1) * 2 * C, 1, r, T.Ip, UL);
+        } else if (g.bc == 1) {
+#pragma unroll
+          for (int v = 0; v < 4; ++v) UL[v] = UW[v];
+        } else {
+#pragma unroll
+          for (int v = 0; v < 4; ++v) UL[v] = __ldg(A.btrW + ((size_t)j * 4 + v) * M + r);
+        }
+        euler_flux<EOS, 0, true>(A.ph, UL, cs2W, cW, FL, lamL);
+        llf(UL, FL, lamL, UW, FWo, lamWo, HW);
+      }
 #pragma unroll
       for (int v = 0; v < 4; ++v)
 #pragma unroll
@@ -271,35 +461,45 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     {
       const int q = w;
       const double xq = xq_col;
+      const double* __restrict__ qn = A.qn + j * row_stride + (size_t)ib * BS + lane;
+      double un[4][M];
+      if (!(A.flags & (F_NO_UN | F_RHS_ONLY))) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+#pragma unroll
+          for (int rr = 0; rr < M; ++rr) un[v][rr] = __ldg(qn + ((v * M + rr) * M + q) * 32);
+      }
       double acc[4][M];
 #pragma unroll
       for (int v = 0; v < 4; ++v)
 #pragma unroll
         for (int r = 0; r < M; ++r) acc[v][r] = 0.0;
-      double US[4] = {0, 0, 0, 0}, UN[4] = {0, 0, 0, 0};
+      double UN[4] = {0, 0, 0, 0}, US[4] = {0, 0, 0, 0};
+      const bool first = !have_HS;
 #pragma unroll
       for (int r = 0; r < M; ++r) {
         double u[4];
 #pragma unroll
-        for (int v = 0; v < 4; ++v) u[v] = __ldg(qb + ((v * M + r) * M + q) * 32);
+        for (int v = 0; v < 4; ++v) u[v] = tu[((v * M + r) * M + q) * 32];
 #pragma unroll
-        for (int v = 0; v < 4; ++v) {
-          US[v] = fma(T.Im[r], u[v], US[v]);
-          UN[v] = fma(T.Ip[r], u[v], UN[v]);
+        for (int v = 0; v < 4; ++v) UN[v] = fma(T.Ip[r], u[v], UN[v]);
+        if (first) {
+#pragma unroll
+          for (int v = 0; v < 4; ++v) US[v] = fma(T.Im[r], u[v], US[v]);
         }
-        const double yr = yc + g.hdy * T.xi[r];
-        // gravity (row a3) and the isothermal sound speed share one rsqrt
+        // gravity (row a3); the isothermal sound speed shares the star's 1/r_s
         double cs2 = 0.0, gx = 0.0, gy = 0.0;
-        if (EOS == 1 || (A.flags & F_GRAV)) {
-          const double ri = rsqrt(fma(xq, xq, fma(yr, yr, A.ph.eps2s)));
+        if (need_ri) {
+          const double yr = yc + g.hdy * T.xi[r];
+          const double ri = sRi[(r * M + q) * 32 + lane];
           if (EOS == 1) cs2 = A.ph.h2gm * ri;
-          if (A.flags & F_GRAV) {
+          if (grav) {
             const double k = -A.ph.gm * ri * ri * ri;
             gx = k * xq;
             gy = k * yr;
             if (A.flags & F_PLANET) {
               const double ddx = xq - A.ph.xp, ddy = yr - A.ph.yp;
-              const double rpi = rsqrt(fma(ddx, ddx, fma(ddy, ddy, A.ph.eps2p)));
+              const double rpi = rsqrt_fast(fma(ddx, ddx, fma(ddy, ddy, A.ph.eps2p)));
               const double kp = -A.ph.qgm * rpi * rpi * rpi;
               gx = fma(kp, ddx, gx);
               gy = fma(kp, ddy, gy);
@@ -307,32 +507,49 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           }
         }
         double G[4], dummy;
-        euler_flux<EOS, 1, false>(A.ph, u, cs2, G, dummy);
+        euler_flux<EOS, 1, false>(A.ph, u, cs2, 0.0, G, dummy);
 #pragma unroll
         for (int v = 0; v < 4; ++v)
 #pragma unroll
           for (int rr = 0; rr < M; ++rr) acc[v][rr] = fma(T.Dy[rr][r], G[v], acc[v][rr]);
-        if (A.flags & F_GRAV) {
+        if (grav) {
           acc[1][r] = fma(u[0], gx, acc[1][r]);
           acc[2][r] = fma(u[0], gy, acc[2][r]);
           acc[3][r] = fma(u[1], gx, fma(u[2], gy, acc[3][r]));
         }
       }
-      // faces: own S/N data; below = carried, above = read ahead from row j+1
-      const double yS = g.y0 + j * g.dy, yN = g.y0 + (j + 1) * g.dy;
-      double GSo[4], GNo[4], lamSo, lamNo;
-      euler_flux<EOS, 1, true>(A.ph, US, cs2_iso<EOS>(A.ph, xq, yS), GSo, lamSo);
-      euler_flux<EOS, 1, true>(A.ph, UN, cs2_iso<EOS>(A.ph, xq, yN), GNo, lamNo);
-      if (bLam < 0.0) {                          // transmissive bottom boundary
+      // south face: carried from the previous row, or built once at the start of the segment
+      if (first) {
+        const double yS = g.y0 + j * g.dy;
+        double cs2 = 0.0, ciso = 0.0;
+        if (EOS == 1) {
+          cs2 = A.ph.h2gm * rsqrt_fast(fma(xq, xq, fma(yS, yS, A.ph.eps2s)));
+          ciso = sqrt_fast(cs2);
+        }
+        double GSo[4], lamSo;
+        euler_flux<EOS, 1, true>(A.ph, US, cs2, ciso, GSo, lamSo);
+        if (!have_below) {                       // transmissive bottom boundary
 #pragma unroll
-        for (int v = 0; v < 4; ++v) { bU[v] = US[v]; bG[v] = GSo[v]; }
-        bLam = lamSo;
+          for (int v = 0; v < 4; ++v) { bU[v] = US[v]; bG[v] = GSo[v]; }
+          bLam = lamSo;
+        }
+        llf(bU, bG, bLam, US, GSo, lamSo, HS);
+        have_HS = true;
       }
+      // north face: own trace against the S trace of the row above (tile t+1)
+      const double yN = g.y0 + (j + 1) * g.dy;
+      double cs2N = 0.0, cN = 0.0;
+      if (EOS == 1) {
+        cs2N = A.ph.h2gm * rsqrt_fast(fma(xq, xq, fma(yN, yN, A.ph.eps2s)));
+        cN = sqrt_fast(cs2N);
+      }
+      double GNo[4], lamNo;
+      euler_flux<EOS, 1, true>(A.ph, UN, cs2N, cN, GNo, lamNo);
       double aU[4], aG[4], aLam;
-      if (j + 1 < g.ny || g.bc == 0) {
-        const int jj = j + 1 < g.ny ? j + 1 : 0;
-        column_trace<M>(A.qprev + jj * row_stride + ib * BS + lane, q, T.Im, aU);
-        euler_flux<EOS, 1, true>(A.ph, aU, cs2_iso<EOS>(A.ph, xq, yN), aG, aLam);
+      if (tile_row(t + 1) >= 0) {
+        tile_wait(t + 1);
+        column_trace<M>(tiles + ((t + 1) % NST) * BS + lane, 32, q, T.Im, aU);
+        euler_flux<EOS, 1, true>(A.ph, aU, cs2N, cN, aG, aLam);
       } else if (g.bc == 1) {
 #pragma unroll
         for (int v = 0; v < 4; ++v) { aU[v] = UN[v]; aG[v] = GNo[v]; }
@@ -340,34 +557,34 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       } else {
 #pragma unroll
         for (int v = 0; v < 4; ++v) aU[v] = __ldg(A.btrN + ((size_t)(ib * 4 + v) * M + q) * 32 + lane);
-        euler_flux<EOS, 1, true>(A.ph, aU, cs2_iso<EOS>(A.ph, xq, yN), aG, aLam);
+        euler_flux<EOS, 1, true>(A.ph, aU, cs2N, cN, aG, aLam);
       }
-      double HS[4], HN[4];
-      llf(bU, bG, bLam, US, GSo, lamSo, HS);
+      double HN[4];
       llf(UN, GNo, lamNo, aU, aG, aLam, HN);
-      // this row's N face becomes the next row's "below"
-#pragma unroll
-      for (int v = 0; v < 4; ++v) { bU[v] = UN[v]; bG[v] = GNo[v]; }
-      bLam = lamNo;
 
-      // wave-killing factors of this cell (row a12)
-      double tau = 0.0;
+      // wave-killing factors of this cell (row a12): out <- f0 u0 + ft out
+      double f0 = 0.0, ft = 1.0;
       bool damp = false;
       if (A.flags & F_DAMP) {
         const double rc = sqrt(xc * xc + yc * yc);
         if (rc > A.damp_r0) {
           const double s = (rc - A.damp_r0) * A.damp_inv_w;
           const double R = fmin(1.0, s * s);
-          if (R > 0.0) { damp = true; tau = A.damp_tau0 / R; }
+          if (R > 0.0) {
+            const double tau = A.damp_tau0 / R;
+            const double inv = 1.0 / (tau + A.dt);
+            damp = true;
+            f0 = A.dt * inv;
+            ft = tau * inv;
+          }
         }
       }
       // modal update in nodal form + RK combination (rows a8, a9) and store
-      double* __restrict__ qo = A.qout + j * row_stride + ib * BS + lane;
-      const double* __restrict__ qn = A.qn + j * row_stride + ib * BS + lane;
-      const double* __restrict__ q0 = A.q0 + j * row_stride + ib * BS + lane;
-      double avg[4] = {0, 0, 0, 0};
+      double* __restrict__ qo = A.qout + j * row_stride + (size_t)ib * BS + lane;
+      const double* __restrict__ q0 = A.q0 + j * row_stride + (size_t)ib * BS + lane;
 #pragma unroll
-      for (int v = 0; v < 4; ++v)
+      for (int v = 0; v < 4; ++v) {
+        double avg = 0.0;
 #pragma unroll
         for (int rr = 0; rr < M; ++rr) {
           const int e = ((v * M + rr) * M + q) * 32;
@@ -376,52 +593,51 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           if (A.flags & F_RHS_ONLY) {
             out = n;
           } else {
-            out = fma(A.dt, n, __ldg(qb + e));
-            if (!(A.flags & F_NO_UN)) out = fma(A.a, __ldg(qn + e), A.b * out);
-            if (damp) out = (A.dt * __ldg(q0 + e) + tau * out) / (tau + A.dt);
+            out = fma(A.dt, n, tu[e]);
+            if (!(A.flags & F_NO_UN)) out = fma(A.a, un[v][rr], A.b * out);
+            if (damp) out = fma(f0, __ldg(q0 + e), ft * out);
           }
           if (valid) qo[e] = out;
-          if (A.flags & F_CFL) avg[v] = fma(T.w[rr], out, avg[v]);
+          avg = fma(T.w[rr], out, avg);
         }
-      // fused CFL wave speed of the state just written (row a10)
-      if (A.flags & F_CFL) {
-        const double wq = 0.25 * T.w[q];
-        if (M > 1) {
-#pragma unroll
-          for (int v = 0; v < 4; ++v) sAvg[(q * 4 + v) * 32 + lane] = wq * avg[v];
-        } else {
-#pragma unroll
-          for (int v = 0; v < 4; ++v) avg[v] *= wq;
-        }
+        if (A.flags & F_CFL) sN[((v * M + 0) * M + q) * 32 + lane] = 0.25 * T.w[q] * avg;
       }
-      __syncthreads();
-      if ((A.flags & F_CFL) && w == 0) {
-        if (M > 1) {
 #pragma unroll
-          for (int v = 0; v < 4; ++v) {
-            double s = 0.0;
-#pragma unroll
-            for (int qq = 0; qq < M; ++qq) s += sAvg[(qq * 4 + v) * 32 + lane];
-            avg[v] = s;
-          }
-        }
-        double sp = 0.0;
-        if (valid) {
-          const double rinv = 1.0 / avg[0];
-          const double vx = avg[1] * rinv, vy = avg[2] * rinv;
-          double c;
-          if (EOS == 0) c = sqrt(A.ph.gamma * A.ph.gm1 * (avg[3] - 0.5 * (avg[1] * vx + avg[2] * vy)) * rinv);
-          else          c = sqrt(cs2_iso<EOS>(A.ph, xc, yc));
-          sp = (fabs(vx) + c) * g.inv_dx + (fabs(vy) + c) * g.inv_dy;
-          if (!(sp >= 0.0)) sp = __longlong_as_double(0x7ff0000000000000LL);   // NaN -> +inf
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) sp = fmax(sp, __shfl_xor_sync(FULL, sp, o));
-        if (lane == 0) atomicMax(A.wmax, (unsigned long long)__double_as_longlong(sp));
-      }
-      // (the sAvg buffer is next written after the following row's first __syncthreads)
+      for (int v = 0; v < 4; ++v) HS[v] = HN[v];   // this row's N face is the next row's S face
+      if (more) edge_store((j + 1) & 1, enext);
     }
+    __syncthreads();
   }
+  // CFL wave speed of the last row of the segment
+  if ((A.flags & F_CFL) && w == 0) {
+    double avg[4];
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+      double s = 0.0;
+#pragma unroll
+      for (int qq = 0; qq < M; ++qq) s += sN[((v * M + 0) * M + qq) * 32 + lane];
+      avg[v] = s;
+    }
+    double sp = 0.0;
+    if (valid) {
+      const double ycp = g.y0 + (j1 - 0.5) * g.dy;
+      const double rinv = 1.0 / avg[0];
+      const double vx = avg[1] * rinv, vy = avg[2] * rinv;
+      double c;
+      if (EOS == 0) c = sqrt(A.ph.gamma * A.ph.gm1 * (avg[3] - 0.5 * (avg[1] * vx + avg[2] * vy)) * rinv);
+      else          c = sqrt(A.ph.h2gm * rsqrt(fma(xc, xc, fma(ycp, ycp, A.ph.eps2s))));
+      sp = (fabs(vx) + c) * g.inv_dx + (fabs(vy) + c) * g.inv_dy;
+      if (!(sp >= 0.0)) sp = __longlong_as_double(0x7ff0000000000000LL);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sp = fmax(sp, __shfl_xor_sync(FULL, sp, o));
+    if (lane == 0) atomicMax(A.wmax, (unsigned long long)__double_as_longlong(sp));
+  }
+}
+
+template <int EOS>
+__device__ __forceinline__ double cs2_iso(const Phys& ph, double x, double y) {
+  return EOS == 1 ? ph.h2gm * rsqrt(fma(x, x, fma(y, y, ph.eps2s))) : 0.0;
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -49,7 +49,7 @@ _lib = None
 def load_library(path: str | None = None):
     """dlopen libdg.so and declare the signatures.  Fails loudly if it has not been built."""
     global _lib
-    if _lib is not None and path is None:
+    if _lib is not None:
         return _lib
     path = path or _LIB_PATH
     if not os.path.exists(path):
