@@ -13,12 +13,15 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdg.so")
-SOURCES = ["dg_api.cu"]
-DEPS = ["dg_api.cu", "dg_kernels.cuh", "dg_tables.h", os.path.join("..", "..", "include", "dg.h")]
-NVCC_FLAGS = [
+SOURCES = ["dg_api.cu"] + [f"dg_stage_m{m}.cu" for m in (1, 2, 3, 4, 5)]
+DEPS = SOURCES + ["dg_kernels.cuh", "dg_stage_launch.cuh", "dg_tables.h",
+                  os.path.join("..", "..", "include", "dg.h")]
+OBJ_DIR = os.path.join(HERE, "build")
+NVCC_COMPILE = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "--extended-lambda", "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+    "--extended-lambda", "-Xcompiler", "-fPIC", "-c",
 ]
+NVCC_LINK = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static"]
 
 
 def needs_build() -> bool:
@@ -28,12 +31,27 @@ def needs_build() -> bool:
     return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if force or needs_build():
-        nvcc = os.environ.get("NVCC", "nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []),
-               *[os.path.join(CSRC, s) for s in SOURCES], "-o", LIB]
-        subprocess.check_call(cmd)
+def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
+    """Compile every translation unit (in parallel) and link libdg.so."""
+    if not (force or needs_build()):
+        return LIB
+    nvcc = os.environ.get("NVCC", "nvcc")
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    procs = []
+    for src in SOURCES:
+        obj = os.path.join(OBJ_DIR, src.replace(".cu", ".o"))
+        cmd = [nvcc, *NVCC_COMPILE, *extra_flags, *(["-Xptxas", "-v"] if verbose else []),
+               os.path.join(CSRC, src), "-o", obj]
+        procs.append((src, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
+    objs = []
+    for src, obj, pr in procs:
+        out, _ = pr.communicate()
+        if verbose or pr.returncode != 0:
+            sys.stderr.write(out)
+        if pr.returncode != 0:
+            raise RuntimeError(f"nvcc failed on {src}")
+        objs.append(obj)
+    subprocess.check_call([nvcc, *NVCC_LINK, *objs, "-o", LIB])
     return LIB
 
 

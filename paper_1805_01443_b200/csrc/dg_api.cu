@@ -13,6 +13,7 @@
 #include "../../include/dg.h"
 #include "dg_tables.h"
 #include "dg_kernels.cuh"
+#include "dg_stage_launch.cuh"
 
 using namespace dg;
 
@@ -110,6 +111,19 @@ int fail(dg_ctx* c, int code, const char* what, cudaError_t e = cudaSuccess) {
     if (e_ != cudaSuccess) return fail((c), DG_ECUDA, #call, e_);    \
   } while (0)
 
+// Register-resident DFMA loop: the fp64 roofline denominator.
+__global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters, double seed) {
+  double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5,
+         a6 = a0 + 6, a7 = a0 + 7;
+  const double m = 0.999999, c = 1e-9;
+  for (int k = 0; k < iters; ++k) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+  if (s == 123.456) out[0] = s;
+}
+
 Phys make_phys(const dg_ctx* c, double t) {
   const dg_params& p = c->p;
   Phys ph{};
@@ -126,27 +140,10 @@ Phys make_phys(const dg_ctx* c, double t) {
   return ph;
 }
 
-template <int M, int EOS>
-void launch_stage_me(dg_ctx* c, const StageArgs& A) {
-  static bool attr_set = false;      // dynamic shared memory above 48 KB must be opted in once
-  constexpr size_t smem = stage_smem_bytes<M>();
-  if (!attr_set) {
-    cudaFuncSetAttribute(stage_kernel<M, EOS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_set = true;
-  }
-  dim3 grid(c->L.nbx, (c->p.ny + A.rows - 1) / A.rows), block(M * 32);
-  stage_kernel<M, EOS><<<grid, block, smem, c->stream>>>(A);
-}
-template <int M>
-int launch_stage_m(dg_ctx* c, const StageArgs& A) {
-  if (c->p.eos == 0) launch_stage_me<M, 0>(c, A);
-  else               launch_stage_me<M, 1>(c, A);
-  return 0;
-}
-
-// One fused stage: qout = a*qn + b*(qprev + dt*L(qprev, t))  (or qout = L when rhs_only).
+// One fused stage: qout = a*qn + b*(qprev + dt*L(qprev, t))  (kind selects the epilogue, K_* in
+// dg_kernels.cuh; K_RHS writes L itself).
 int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout, double a, double b,
-                 double dt, double t, int flags) {
+                 double dt, double t, int kind) {
   StageArgs A{};
   A.qprev = qprev; A.qn = qn; A.qout = qout; A.q0 = c->q0();
   A.btrW = c->btrW(); A.btrE = c->btrE(); A.btrS = c->btrS(); A.btrN = c->btrN();
@@ -158,27 +155,27 @@ int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout,
       ? 2.0 * 3.14159265358979323846 * std::sqrt(c->p.damp_r0 * c->p.damp_r0 * c->p.damp_r0 / c->p.gm_star)
       : 0.0;
   A.rows = c->rows_per_cta;
-  if (c->p.gm_star > 0.0) flags |= F_GRAV;
-  if (c->p.gm_star > 0.0 && c->p.q_planet > 0.0) flags |= F_PLANET;
-  A.flags = flags;
   A.g = c->g;
   A.ph = make_phys(c, t);
   A.T = c->T;
+  const int grav = c->p.gm_star > 0.0 ? (c->p.q_planet > 0.0 ? G_PLANET : G_STAR) : G_NONE;
+  dim3 grid(c->L.nbx, (c->p.ny + A.rows - 1) / A.rows);
   const bool timed = c->timing && c->ev_used + 2 <= c->evs.size();
   if (timed) cudaEventRecord(c->evs[c->ev_used], c->stream);
+  cudaError_t e;
   switch (c->L.m) {
-    case 1: launch_stage_m<1>(c, A); break;
-    case 2: launch_stage_m<2>(c, A); break;
-    case 3: launch_stage_m<3>(c, A); break;
-    case 4: launch_stage_m<4>(c, A); break;
-    default: launch_stage_m<5>(c, A); break;
+    case 1: e = launch_stage_m1(A, c->p.eos, grav, kind, grid, c->stream); break;
+    case 2: e = launch_stage_m2(A, c->p.eos, grav, kind, grid, c->stream); break;
+    case 3: e = launch_stage_m3(A, c->p.eos, grav, kind, grid, c->stream); break;
+    case 4: e = launch_stage_m4(A, c->p.eos, grav, kind, grid, c->stream); break;
+    default: e = launch_stage_m5(A, c->p.eos, grav, kind, grid, c->stream); break;
   }
   c->launches++;
   if (timed) {
     cudaEventRecord(c->evs[c->ev_used + 1], c->stream);
     c->ev_used += 2;
   }
-  CUDA_TRY(c, cudaGetLastError());
+  if (e != cudaSuccess) return fail(c, DG_ECUDA, "stage kernel launch", e);
   return DG_OK;
 }
 
@@ -268,26 +265,28 @@ int do_step(dg_ctx* c, double dt, double* stages) {
   const int A = c->cur, B = (c->cur + 1) % 3, Cc = (c->cur + 2) % 3;
   const size_t n = (size_t)c->p.ny * c->p.nx * 4 * c->L.m * c->L.m;
   const bool damp = c->p.damp_r0 > 0.0;
-  int last = (damp ? F_DAMP : 0) | (c->fused_cfl ? F_CFL : 0);
-  if (stages) last = 0;      // debug stages are "before damping": damping runs as its own pass below
+  // the fused reduction rides on the last stage (K_LAST*); with DG_TUNE_FUSED_CFL = 0 or in the debug
+  // path (stages are "before damping": damping runs as its own pass below) the last stage is plain
+  int last = damp ? K_LASTD : K_LAST;
+  if (stages || (!c->fused_cfl && !damp)) last = K_MID;
   int e;
   if (c->fused_cfl && !stages)
     CUDA_TRY(c, cudaMemsetAsync(c->wmax(), 0, sizeof(unsigned long long), c->stream));
   // SSP-RK in Shu-Osher form, stage times c = (0,1) / (0,1,1/2)
-  if ((e = launch_stage(c, c->q(A), c->q(A), c->q(B), 0.0, 1.0, dt, c->t, F_NO_UN))) return e;
+  if ((e = launch_stage(c, c->q(A), c->q(A), c->q(B), 0.0, 1.0, dt, c->t, K_FIRST))) return e;
   if (stages && (e = to_modal(c, c->q(B), stages))) return e;
   if (c->p.rk == 2) {
     if ((e = launch_stage(c, c->q(B), c->q(A), c->q(Cc), 0.5, 0.5, dt, c->t + dt, last))) return e;
     if (stages && (e = to_modal(c, c->q(Cc), stages + n))) return e;
     c->cur = Cc;
   } else {
-    if ((e = launch_stage(c, c->q(B), c->q(A), c->q(Cc), 0.75, 0.25, dt, c->t + dt, 0))) return e;
+    if ((e = launch_stage(c, c->q(B), c->q(A), c->q(Cc), 0.75, 0.25, dt, c->t + dt, K_MID))) return e;
     if (stages && (e = to_modal(c, c->q(Cc), stages + n))) return e;
     if ((e = launch_stage(c, c->q(Cc), c->q(A), c->q(B), 1.0 / 3.0, 2.0 / 3.0, dt, c->t + 0.5 * dt, last))) return e;
     if (stages && (e = to_modal(c, c->q(B), stages + 2 * n))) return e;
     c->cur = B;
   }
-  c->wmax_valid = c->fused_cfl && !stages;
+  c->wmax_valid = c->fused_cfl && last >= K_LAST;
   if (stages && damp) {   // debug path: stages are "before damping", so relax in a separate pass
     if ((e = launch_damp(c, c->q(c->cur), dt))) return e;
   }
@@ -392,7 +391,7 @@ int dg_rhs(dg_ctx* c, double t, double* Lout) {
   if (!c || !Lout) return c ? fail(c, DG_EINVAL, "dg_rhs: null") : DG_EINVAL;
   if (!c->has_state) return fail(c, DG_ESTATE, "dg_rhs: state not set");
   double* scratch = c->q((c->cur + 1) % 3);
-  int e = launch_stage(c, c->q(c->cur), c->q(c->cur), scratch, 0.0, 1.0, 0.0, t, F_RHS_ONLY | F_NO_UN);
+  int e = launch_stage(c, c->q(c->cur), c->q(c->cur), scratch, 0.0, 1.0, 0.0, t, K_RHS);
   if (e) return e;
   return to_modal(c, scratch, Lout);
 }

@@ -23,14 +23,17 @@ namespace dg {
 
 constexpr unsigned FULL = 0xffffffffu;
 
-enum : int {
-  F_RHS_ONLY = 1,   // write N = L(u) instead of the RK combination
-  F_NO_UN    = 2,   // alpha = 0: do not read u^n
-  F_DAMP     = 4,   // apply the wave-killing relaxation after the combination (last stage)
-  F_CFL      = 8,   // reduce the CFL wave speed of the written state
-  F_GRAV     = 16,
-  F_PLANET   = 32,
+// Kernel variants are compile-time so that the unrolled node loops are straight-line code (runtime
+// flags inside them split basic blocks and stop the scheduler from interleaving the nodes' chains).
+enum : int {          // KIND: what the epilogue of the stage does
+  K_RHS   = 0,        // write N = L(u)                                   (dg_rhs)
+  K_FIRST = 1,        // u + dt N                                         (stage 1: alpha = 0, u^n not read)
+  K_MID   = 2,        // a u^n + b (u + dt N)
+  K_LAST  = 3,        // K_MID + fused CFL wave-speed reduction
+  K_LASTD = 4,        // K_LAST + wave-killing relaxation
+  K_COUNT = 5,
 };
+enum : int { G_NONE = 0, G_STAR = 1, G_PLANET = 2 };   // GRAV: gravity source terms present
 
 struct DevTables {            // kernel-parameter (constant bank) copy of the tables
   double xi[MAXM], w[MAXM];
@@ -63,7 +66,7 @@ struct StageArgs {
   unsigned long long* wmax;   // CFL wave-speed maximum (bit pattern of a non-negative double)
   double a, b, dt;
   double damp_r0, damp_inv_w, damp_tau0;
-  int rows, flags;
+  int rows;
   Geom g;
   Phys ph;
   DevTables T;
@@ -76,18 +79,14 @@ struct StageArgs {
 __device__ __forceinline__ double rcp_fast(double x) {
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
-  e = fma(-x, r, 1.0);
-  return fma(r, e, r);
+  const double e = fma(-x, r, 1.0);             // r <- r (1 + e + e^2), e ~ 1e-6
+  return fma(r, fma(e, e, e), r);
 }
 __device__ __forceinline__ double rsqrt_fast(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double e = fma(-(x * y), y, 1.0);
-  y = fma(0.5 * y, e, y);
-  e = fma(-(x * y), y, 1.0);
-  return fma(0.5 * y, e, y);
+  const double e = fma(-(x * y), y, 1.0);        // y <- y (1 + e/2 + 3 e^2/8), e ~ 1e-6
+  return fma(y, e * fma(0.375, e, 0.5), y);
 }
 __device__ __forceinline__ double sqrt_fast(double x) { return x * rsqrt_fast(x); }
 
@@ -195,9 +194,6 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 //   sRi       1/sqrt(x^2+y^2+eps^2) at the row's volume nodes (shared by c_s^2 and the star gravity)
 //   sEdge[2]  the two x-neighbour cells outside the block, prefetched one row ahead
 // ---------------------------------------------------------------------------------------------
-#ifndef DG_STAGE_MINB
-#define DG_STAGE_MINB 2
-#endif
 constexpr int NST = 3;
 
 template <int M>
@@ -206,9 +202,14 @@ constexpr size_t stage_smem_bytes() {
   return ((size_t)(NST + 1) * 4 * M * M * 32 + (size_t)M * M * 32 + (size_t)4 * 4 * M * M) * sizeof(double) + 64;
 }
 
-template <int M, int EOS>
-__global__ void __launch_bounds__(M * 32, DG_STAGE_MINB)
+template <int M, int EOS, int GRAV, int KIND, int MINB>
+__global__ void __launch_bounds__(M * 32, MINB)
 stage_kernel(const __grid_constant__ StageArgs A) {
+  constexpr bool grav = GRAV != G_NONE;
+  constexpr bool need_ri = EOS == 1 || grav;
+  constexpr bool use_un = KIND >= K_MID;
+  constexpr bool do_cfl = KIND >= K_LAST;
+  constexpr bool do_damp = KIND == K_LASTD;
   constexpr int C = 4 * M * M;                   // doubles per cell
   constexpr int BS = C * 32;                     // doubles per 32-cell tile
   constexpr int NT = M * 32;
@@ -232,8 +233,6 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   const int j0 = blockIdx.y * A.rows;
   const int j1 = min(g.ny, j0 + A.rows);
   const size_t row_stride = (size_t)g.nbx * BS;
-  const bool grav = (A.flags & F_GRAV) != 0;
-  const bool need_ri = EOS == 1 || grav;
 
   const double xc = g.x0 + (i + 0.5) * g.dx;
   const double xW = g.x0 + i * g.dx, xE = g.x0 + (i + 1) * g.dx;
@@ -305,6 +304,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   // numerical flux through the south face of the row about to be processed, column q = w
   double HS[4];
   bool have_HS = false;
+  double spmax = 0.0;                            // running CFL wave-speed maximum of this lane (warp 0)
   double bU[4], bG[4], bLam = 0.0;               // north-face data of the row below (first row only)
   bool have_below = false;
   {
@@ -338,7 +338,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 
     // fused CFL wave speed of the row finished in the previous iteration (row a10).
     // Partial cell averages were parked in sN[v][r=0][q][lane], which only this warp rewrites.
-    if ((A.flags & F_CFL) && w == 0 && j > j0) {
+    if (do_cfl && w == 0 && j > j0) {
       double avg[4];
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
@@ -358,9 +358,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
         sp = (fabs(vx) + c) * g.inv_dx + (fabs(vy) + c) * g.inv_dy;
         if (!(sp >= 0.0)) sp = __longlong_as_double(0x7ff0000000000000LL);   // NaN -> +inf
       }
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) sp = fmax(sp, __shfl_xor_sync(FULL, sp, o));
-      if (lane == 0) atomicMax(A.wmax, (unsigned long long)__double_as_longlong(sp));
+      spmax = fmax(spmax, sp);                   // per lane; reduced once after the last row
     }
 
     tile_wait(t);
@@ -463,7 +461,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       const double xq = xq_col;
       const double* __restrict__ qn = A.qn + j * row_stride + (size_t)ib * BS + lane;
       double un[4][M];
-      if (!(A.flags & (F_NO_UN | F_RHS_ONLY))) {
+      if (use_un) {
 #pragma unroll
         for (int v = 0; v < 4; ++v)
 #pragma unroll
@@ -474,7 +472,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       for (int v = 0; v < 4; ++v)
 #pragma unroll
         for (int r = 0; r < M; ++r) acc[v][r] = 0.0;
-      double UN[4] = {0, 0, 0, 0}, US[4] = {0, 0, 0, 0};
+      double UN[4] = {0, 0, 0, 0};
       const bool first = !have_HS;
 #pragma unroll
       for (int r = 0; r < M; ++r) {
@@ -483,10 +481,6 @@ stage_kernel(const __grid_constant__ StageArgs A) {
         for (int v = 0; v < 4; ++v) u[v] = tu[((v * M + r) * M + q) * 32];
 #pragma unroll
         for (int v = 0; v < 4; ++v) UN[v] = fma(T.Ip[r], u[v], UN[v]);
-        if (first) {
-#pragma unroll
-          for (int v = 0; v < 4; ++v) US[v] = fma(T.Im[r], u[v], US[v]);
-        }
         // gravity (row a3); the isothermal sound speed shares the star's 1/r_s
         double cs2 = 0.0, gx = 0.0, gy = 0.0;
         if (need_ri) {
@@ -497,7 +491,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
             const double k = -A.ph.gm * ri * ri * ri;
             gx = k * xq;
             gy = k * yr;
-            if (A.flags & F_PLANET) {
+            if (GRAV == G_PLANET) {
               const double ddx = xq - A.ph.xp, ddy = yr - A.ph.yp;
               const double rpi = rsqrt_fast(fma(ddx, ddx, fma(ddy, ddy, A.ph.eps2p)));
               const double kp = -A.ph.qgm * rpi * rpi * rpi;
@@ -520,6 +514,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       }
       // south face: carried from the previous row, or built once at the start of the segment
       if (first) {
+        double US[4];
+        column_trace<M>(tu, 32, q, T.Im, US);
         const double yS = g.y0 + j * g.dy;
         double cs2 = 0.0, ciso = 0.0;
         if (EOS == 1) {
@@ -565,7 +561,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       // wave-killing factors of this cell (row a12): out <- f0 u0 + ft out
       double f0 = 0.0, ft = 1.0;
       bool damp = false;
-      if (A.flags & F_DAMP) {
+      if (do_damp) {
         const double rc = sqrt(xc * xc + yc * yc);
         if (rc > A.damp_r0) {
           const double s = (rc - A.damp_r0) * A.damp_inv_w;
@@ -590,17 +586,17 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           const int e = ((v * M + rr) * M + q) * 32;
           const double n = sN[e + lane] + fma(T.lym[rr], HS[v], fma(-T.lyp[rr], HN[v], acc[v][rr]));
           double out;
-          if (A.flags & F_RHS_ONLY) {
+          if (KIND == K_RHS) {
             out = n;
           } else {
             out = fma(A.dt, n, tu[e]);
-            if (!(A.flags & F_NO_UN)) out = fma(A.a, un[v][rr], A.b * out);
-            if (damp) out = fma(f0, __ldg(q0 + e), ft * out);
+            if (use_un) out = fma(A.a, un[v][rr], A.b * out);
+            if (do_damp && damp) out = fma(f0, __ldg(q0 + e), ft * out);
           }
           if (valid) qo[e] = out;
-          avg = fma(T.w[rr], out, avg);
+          if (do_cfl) avg = fma(T.w[rr], out, avg);
         }
-        if (A.flags & F_CFL) sN[((v * M + 0) * M + q) * 32 + lane] = 0.25 * T.w[q] * avg;
+        if (do_cfl) sN[((v * M + 0) * M + q) * 32 + lane] = 0.25 * T.w[q] * avg;
       }
 #pragma unroll
       for (int v = 0; v < 4; ++v) HS[v] = HN[v];   // this row's N face is the next row's S face
@@ -608,8 +604,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     }
     __syncthreads();
   }
-  // CFL wave speed of the last row of the segment
-  if ((A.flags & F_CFL) && w == 0) {
+  // CFL wave speed of the last row of the segment, then one reduction per thread block
+  if (do_cfl && w == 0) {
     double avg[4];
 #pragma unroll
     for (int v = 0; v < 4; ++v) {
@@ -629,9 +625,14 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       sp = (fabs(vx) + c) * g.inv_dx + (fabs(vy) + c) * g.inv_dy;
       if (!(sp >= 0.0)) sp = __longlong_as_double(0x7ff0000000000000LL);
     }
+    // non-negative doubles order like their bit patterns
+    unsigned long long bits = (unsigned long long)__double_as_longlong(fmax(spmax, sp));
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) sp = fmax(sp, __shfl_xor_sync(FULL, sp, o));
-    if (lane == 0) atomicMax(A.wmax, (unsigned long long)__double_as_longlong(sp));
+    for (int o = 16; o > 0; o >>= 1) {
+      const unsigned long long other = __shfl_xor_sync(FULL, bits, o);
+      bits = other > bits ? other : bits;
+    }
+    if (lane == 0) atomicMax(A.wmax, bits);
   }
 }
 
@@ -825,19 +826,6 @@ damp_kernel(double* __restrict__ Q, const double* __restrict__ Q0, Geom g, doubl
   const size_t base = ((size_t)j * g.nbx + ib) * C * 32 + lane;
 #pragma unroll 4
   for (int e = 0; e < C; ++e) Q[base + e * 32] = (dt * Q0[base + e * 32] + tau * Q[base + e * 32]) / (tau + dt);
-}
-
-// Register-resident DFMA loop: the fp64 roofline denominator.
-__global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters, double seed) {
-  double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5,
-         a6 = a0 + 6, a7 = a0 + 7;
-  const double m = 0.999999, c = 1e-9;
-  for (int k = 0; k < iters; ++k) {
-    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
-    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
-  }
-  const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
-  if (s == 123.456) out[0] = s;
 }
 
 }  // namespace dg
