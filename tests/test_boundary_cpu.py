@@ -1,0 +1,163 @@
+"""CPU-side checks of the boundary (no compute calls): libdg.so builds with nvcc for sm_100a, loads,
+exports every symbol include/dg.h declares, validates parameters and sizes the workspace; the
+Python binding mirrors dg_params field by field; the product fails loudly without a GPU; nothing
+in the product package imports the oracle."""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "dg.h")
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1805_01443_b200.build import build
+    from paper_1805_01443_b200.dg import load_library
+    build()
+    return load_library()
+
+
+def _declared_functions():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(dg_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    from paper_1805_01443_b200.dg import EXPORTS
+    declared = _declared_functions()
+    assert len(declared) >= 15
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in include/dg.h but not exported by libdg.so"
+    assert sorted(EXPORTS) == declared, "binding's EXPORTS list and the header disagree"
+
+
+def test_binding_struct_matches_header():
+    from paper_1805_01443_b200.dg import DGParams
+    src = open(HEADER).read()
+    body = src[src.index("typedef struct {"):src.index("} dg_params;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = []
+    for typ, names in re.findall(r"\b(int32_t|double)\s+([^;]+);", body):
+        for nm in names.split(","):
+            fields.append((nm.strip(), C.c_int32 if typ == "int32_t" else C.c_double))
+    assert [(n, t) for n, t in DGParams._fields_] == fields
+
+
+def test_workspace_sizing_and_validation(lib):
+    from paper_1805_01443_b200 import workloads as W
+    from paper_1805_01443_b200.dg import params_struct
+    p, _ = W.vortex(32, 2)
+    n = lib.dg_workspace_bytes(C.byref(params_struct(p)))
+    state = 32 * 32 * 4 * 4 * 8
+    assert 3 * state <= n < 3 * state + 4096            # three state buffers + scalars, periodic: no snapshot
+    pd, _ = W.disc(33, 3, planet=True)
+    nd = lib.dg_workspace_bytes(C.byref(params_struct(pd)))
+    padded = 33 * 64 * 4 * 9 * 8                        # x padded to whole 32-cell blocks
+    assert nd >= 4 * padded                             # + snapshot of the initial state (bc 2 / damping)
+    for bad in (dict(order=0), dict(order=6), dict(rk=4), dict(bc=3), dict(eos=2), dict(nx=0),
+                dict(x1=p["x0"]), dict(gamma=1.0), dict(eos=1), dict(damp_r0=1.0, damp_r1=0.5)):
+        assert lib.dg_workspace_bytes(C.byref(params_struct(dict(p, **bad)))) == 0, bad
+    assert lib.dg_workspace_bytes(None) == 0
+    h = C.c_void_p()
+    assert lib.dg_init(C.byref(params_struct(p)), None, n, None, C.byref(h)) == -1
+    assert lib.dg_init(C.byref(params_struct(p)), C.c_void_p(256), n, None, None) == -1
+    assert lib.dg_last_error(None) == b"null context"
+    lib.dg_destroy(None)
+
+
+def test_no_cpu_fallback():
+    """Without a device the product refuses to run (it must not route through the oracle)."""
+    import torch
+    from paper_1805_01443_b200 import DG, DGError, workloads as W
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is visible")
+    p, _ = W.vortex(8, 2)
+    with pytest.raises(DGError):
+        DG(p)
+
+
+def test_product_never_imports_oracle():
+    pkg = os.path.join(ROOT, "paper_1805_01443_b200")
+    for dirpath, _dirs, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert "ref_dg" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp", ".h")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(import|from)\s+paper_1805_01443_b200\b", txt, flags=re.M), f
+            for inc in re.findall(r'#include\s+"([^"]+)"', txt):
+                assert os.path.basename(inc) in ("ref_dg.h",), (f, inc)
+
+
+def test_sass_uses_bulk_async_copy():
+    """The stage kernel's tile ring is fed by TMA bulk copies (UBLKCP in SASS) and waits on mbarriers."""
+    from paper_1805_01443_b200.build import LIB, build
+    build()
+    out = subprocess.run(["cuobjdump", "-sass", "-fun", "stage_kernel", LIB], capture_output=True, text=True)
+    if out.returncode != 0 or "UBLKCP" not in out.stdout:
+        out = subprocess.run(["cuobjdump", "-sass", LIB], capture_output=True, text=True)
+    assert "UBLKCP" in out.stdout
+    assert "SYNCS" in out.stdout          # mbarrier arrive / try_wait
+
+
+def _gloo_worker(rank, size, port, q):
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(size),
+                      MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    sys.path.insert(0, ROOT)
+    from paper_1805_01443_b200 import replicas
+    assert replicas.world() == (rank, rank, size)
+    assert replicas.init("gloo")
+    replicas.barrier()
+    # rank r took (10 + 5 r) ms for 1000 units: the job did 2000 units in max = 15 ms
+    value, t = replicas.throughput(10.0 + 5.0 * rank, 1000.0)
+    replicas.barrier()
+    replicas.finish()
+    q.put((rank, value, t))
+
+
+def test_replicas_aggregation_gloo_world2():
+    """The only cross-rank logic of bench.py --gpus N: barrier, max time, summed units (gloo, 2 ranks)."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_gloo_worker, args=(r, 2, port, q)) for r in range(2)]
+    for pr in procs:
+        pr.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for pr in procs:
+        pr.join(timeout=60)
+        assert pr.exitcode == 0
+    for _rank, value, t in res:
+        assert t == 15.0
+        assert abs(value - 2000.0 / 15e-3) < 1e-6
+
+
+def test_replicas_single_process_passthrough():
+    from paper_1805_01443_b200 import replicas
+    assert replicas.throughput(4.0, 8.0) == (2000.0, 4.0)
+
+
+def test_bench_accounting():
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1805_01443_b200 import workloads as W
+    p = W.make_params(nx=1024, ny=1024, order=5, rk=3, x0=-2.5, x1=2.5, y0=-2.5, y1=2.5, damp_r0=2.2, damp_r1=2.5,
+                      gm_star=1.0)
+    bpl, acct = bench.stage_bytes_per_launch(p)
+    state = 1024 * 1024 * 100 * 8
+    f = 1.0 - np.pi * 2.2 ** 2 / 25.0
+    assert acct["state_bytes"] == state
+    assert abs(acct["damping_zone_fraction"] - f) < 2e-3
+    assert abs(bpl - state * (8 + f) / 3) < 1e-3 * state
+    assert bpl / (1024 * 1024 * 25) <= 96.0             # never above SURVEY's 96 B per DOF-update
