@@ -121,6 +121,8 @@ int dg_set_tuning(dg_ctx*, int key, int value);
  * the number of launches measured (synchronises). */
 int dg_stage_timing(dg_ctx*, int enable);
 int dg_stage_time_ms(dg_ctx*, double* mean_ms /*HOST*/, long long* launches /*HOST*/);
+/* The individual durations (ms) of up to `capacity` measured stage launches, in launch order (synchronises). */
+int dg_stage_times_ms(dg_ctx*, double* ms /*HOST, capacity doubles*/, long long capacity, long long* launches /*HOST*/);
 
 /* Diagnostic: sustained fp64 FMA throughput of this GPU (register-resident DFMA loop),
  * TFLOP/s counting an FMA as 2 flops.  Uses the context's stream; blocking. */

@@ -494,6 +494,19 @@ int dg_stage_time_ms(dg_ctx* c, double* mean_ms, long long* launches) {
   return DG_OK;
 }
 
+int dg_stage_times_ms(dg_ctx* c, double* ms, long long capacity, long long* launches) {
+  if (!c || !ms || !launches || capacity < 0) return DG_EINVAL;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  long long n = 0;
+  for (size_t k = 0; k + 1 < c->ev_used && n < capacity; k += 2, ++n) {
+    float t = 0.f;
+    CUDA_TRY(c, cudaEventElapsedTime(&t, c->evs[k], c->evs[k + 1]));
+    ms[n] = t;
+  }
+  *launches = n;
+  return DG_OK;
+}
+
 int dg_probe_fp64_peak(dg_ctx* c, double* tflops) {
   if (!c || !tflops) return DG_EINVAL;
   int dev = 0, sms = 0;

@@ -14,7 +14,7 @@ EXPORTS = [
     "dg_workspace_bytes", "dg_init", "dg_set_state", "dg_set_state_host", "dg_get_state",
     "dg_get_state_host", "dg_rhs", "dg_cfl_dt", "dg_step", "dg_step_debug", "dg_run_host",
     "dg_time", "dg_set_time", "dg_launch_count", "dg_set_tuning", "dg_stage_timing",
-    "dg_stage_time_ms", "dg_probe_fp64_peak", "dg_last_error", "dg_destroy",
+    "dg_stage_time_ms", "dg_stage_times_ms", "dg_probe_fp64_peak", "dg_last_error", "dg_destroy",
 ]
 
 
@@ -72,6 +72,7 @@ def load_library(path: str | None = None):
         "dg_set_tuning": (i, [vp, i, i]),
         "dg_stage_timing": (i, [vp, i]),
         "dg_stage_time_ms": (i, [vp, C.POINTER(d), C.POINTER(ll)]),
+        "dg_stage_times_ms": (i, [vp, C.POINTER(d), ll, C.POINTER(ll)]),
         "dg_probe_fp64_peak": (i, [vp, C.POINTER(d)]),
         "dg_last_error": (C.c_char_p, [vp]),
         "dg_destroy": (None, [vp]),
@@ -205,6 +206,11 @@ class DG:
         ms, n = C.c_double(), C.c_longlong()
         self._chk(self.L.dg_stage_time_ms(self._h, C.byref(ms), C.byref(n)), "dg_stage_time_ms")
         return ms.value, n.value
+
+    def stage_times_ms(self, capacity: int = 4096):
+        buf, n = (C.c_double * capacity)(), C.c_longlong()
+        self._chk(self.L.dg_stage_times_ms(self._h, buf, capacity, C.byref(n)), "dg_stage_times_ms")
+        return list(buf[:n.value])
 
     def probe_fp64_peak(self) -> float:
         tf = C.c_double()
