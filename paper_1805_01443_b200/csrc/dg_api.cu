@@ -124,15 +124,16 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters,
   if (s == 123.456) out[0] = s;
 }
 
-Phys make_phys(const dg_ctx* c, double t) {
+// beta: the factor of N in the stage's output, folded into the gravity constants (and the tables)
+Phys make_phys(const dg_ctx* c, double t, double beta = 1.0) {
   const dg_params& p = c->p;
   Phys ph{};
   ph.gamma = p.gamma;
   ph.gm1 = p.gamma - 1.0;
   ph.h2gm = p.h_aspect * p.h_aspect * p.gm_star;
-  ph.gm = p.gm_star;
+  ph.gmb = beta * p.gm_star;
   ph.eps2s = p.eps_star * p.eps_star;
-  ph.qgm = p.q_planet * p.gm_star;
+  ph.qgmb = beta * p.q_planet * p.gm_star;
   const double ang = p.omega_planet * t + p.phase0;
   ph.xp = p.r_planet * std::cos(ang);
   ph.yp = p.r_planet * std::sin(ang);
@@ -141,10 +142,13 @@ Phys make_phys(const dg_ctx* c, double t) {
 }
 
 // One fused stage: qout = a*qn + b*(qprev + dt*L(qprev, t))  (kind selects the epilogue, K_* in
-// dg_kernels.cuh; K_RHS writes L itself).
+// dg_kernels.cuh; K_RHS writes L itself).  The kernel computes a*qn + b*qprev + beta*L with
+// beta = b*dt folded into the derivative / lifting tables and the gravity constants here; the
+// lifting vectors also carry the 1/2 of the Lax-Friedrichs average (the kernel forms 2 x flux).
 int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout, double a, double b,
                  double dt, double t, int kind) {
   StageArgs A{};
+  const double beta = kind == K_RHS ? 1.0 : b * dt;
   A.qprev = qprev; A.qn = qn; A.qout = qout; A.q0 = c->q0();
   A.btrW = c->btrW(); A.btrE = c->btrE(); A.btrS = c->btrS(); A.btrN = c->btrN();
   A.wmax = c->wmax();
@@ -156,8 +160,12 @@ int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout,
       : 0.0;
   A.rows = c->rows_per_cta;
   A.g = c->g;
-  A.ph = make_phys(c, t);
+  A.ph = make_phys(c, t, beta);
   A.T = c->T;
+  for (int q = 0; q < c->L.m; ++q) {
+    A.T.lxp[q] *= 0.5 * beta; A.T.lxm[q] *= 0.5 * beta; A.T.lyp[q] *= 0.5 * beta; A.T.lym[q] *= 0.5 * beta;
+    for (int k = 0; k < c->L.m; ++k) { A.T.Dx[q][k] *= beta; A.T.Dy[q][k] *= beta; }
+  }
   const int grav = c->p.gm_star > 0.0 ? (c->p.q_planet > 0.0 ? G_PLANET : G_STAR) : G_NONE;
   dim3 grid(c->L.nbx, (c->p.ny + A.rows - 1) / A.rows);
   const bool timed = c->timing && c->ev_used + 2 <= c->evs.size();

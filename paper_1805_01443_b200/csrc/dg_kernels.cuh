@@ -37,9 +37,9 @@ enum : int { G_NONE = 0, G_STAR = 1, G_PLANET = 2 };   // GRAV: gravity source t
 
 struct DevTables {            // kernel-parameter (constant bank) copy of the tables
   double xi[MAXM], w[MAXM];
-  double Dx[MAXM][MAXM];      // Dh[q'][q]/dx
-  double Dy[MAXM][MAXM];      // Dh[r'][r]/dy
-  double lxp[MAXM], lxm[MAXM], lyp[MAXM], lym[MAXM];   // lift vectors / dx, / dy
+  double Dx[MAXM][MAXM];      // beta Dh[q'][q]/dx
+  double Dy[MAXM][MAXM];      // beta Dh[r'][r]/dy
+  double lxp[MAXM], lxm[MAXM], lyp[MAXM], lym[MAXM];   // (beta/2) lift vectors / dx, / dy (kernels carry 2 x LLF flux)
   double Ip[MAXM], Im[MAXM];  // interpolation to xi = +1 / -1
 };
 
@@ -48,8 +48,8 @@ struct ConvTables { double B[MAXM][MAXM], P[MAXM][MAXM]; };
 struct Phys {
   double gamma, gm1;          // eos 0
   double h2gm;                // eos 1: h^2 GM
-  double gm, eps2s;           // star
-  double qgm, xp, yp, eps2p;  // planet at the stage time
+  double gmb, eps2s;          // star: beta GM (beta = the stage's factor of N, folded in on the host)
+  double qgmb, xp, yp, eps2p; // planet at the stage time: beta q GM
 };
 
 struct Geom {
@@ -64,7 +64,7 @@ struct StageArgs {
   const double* q0;           // initial state (damping)
   const double* btrW; const double* btrE; const double* btrS; const double* btrN;  // bc 2 traces
   unsigned long long* wmax;   // CFL wave-speed maximum (bit pattern of a non-negative double)
-  double a, b, dt;
+  double a, b, dt;            // out = a u^n + b u^(s-1) + beta N; beta = b dt is folded into T and ph
   double damp_r0, damp_inv_w, damp_tau0;
   int rows;
   Geom g;
@@ -115,31 +115,21 @@ __device__ __forceinline__ void euler_flux(const Phys& ph, const double (&u)[4],
   }
 }
 
-// Local Lax-Friedrichs flux from the two sides' states, fluxes and speeds.
+// Local Lax-Friedrichs flux from the two sides' states, fluxes and speeds,
+// TIMES TWO: (FL + FR) - max(lamL, lamR) (UR - UL); the 1/2 lives in the lifting tables.
 // Each interior face is evaluated exactly once (by the cell on its left / below) and handed to the
 // other cell, so the interface flux is single valued to the last bit.
-__device__ __forceinline__ void llf(const double (&UL)[4], const double (&FL)[4], double lamL,
-                                    const double (&UR)[4], const double (&FR)[4], double lamR,
-                                    double (&H)[4]) {
-  const double hl = 0.5 * fmax(lamL, lamR);
+__device__ __forceinline__ void llf2(const double (&UL)[4], const double (&FL)[4], double lamL,
+                                     const double (&UR)[4], const double (&FR)[4], double lamR,
+                                     double (&H)[4]) {
+  const double lam = fmax(lamL, lamR);
 #pragma unroll
-  for (int v = 0; v < 4; ++v) H[v] = fma(-hl, UR[v] - UL[v], 0.5 * (FL[v] + FR[v]));
+  for (int v = 0; v < 4; ++v) H[v] = fma(-lam, UR[v] - UL[v], FL[v] + FR[v]);
 }
 
 // ---------------------------------------------------------------------------------------------
-// Traces of a cell (node stride `s` doubles: 32 inside a tile, 1 inside the edge buffer)
+// Trace of a cell at eta = -1/+1 (node stride `s` doubles: 32 inside a tile)
 // ---------------------------------------------------------------------------------------------
-template <int M>
-__device__ __forceinline__ void line_trace(const double* cell, int stride, int r,
-                                           const double (&I)[MAXM], double (&out)[4]) {
-#pragma unroll
-  for (int v = 0; v < 4; ++v) {
-    double s = 0.0;
-#pragma unroll
-    for (int q = 0; q < M; ++q) s = fma(I[q], cell[((v * M + r) * M + q) * stride], s);
-    out[v] = s;
-  }
-}
 template <int M>
 __device__ __forceinline__ void column_trace(const double* cell, int stride, int q,
                                              const double (&I)[MAXM], double (&out)[4]) {
@@ -181,25 +171,37 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+// orders earlier generic-proxy accesses of shared memory before later async-proxy (TMA) writes
+__device__ __forceinline__ void fence_proxy_async() {
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
 // ---------------------------------------------------------------------------------------------
 // The fused RK-stage kernel (rows a2..a12 of SURVEY.md 8(a); a1/a4's basis change is folded into
-// the tables, see dg_tables.h).
+// the tables, see dg_tables.h).  Writes
+//     out = a u^n + b u^(s-1) + beta N(u^(s-1)),     beta = b dt,
+// with beta (and the 1/2 of the Lax-Friedrichs average) folded into the derivative / lifting tables
+// and the gravity constants on the host; K_RHS: a = b = 0, beta = 1.
 //
 // Shared memory of one thread block (M warps, one 32-cell column block, `rows` rows):
 //   tiles[3]  ring of u^(s-1) tiles (rows j-1 | j | j+1 | j+2 rotating), each one contiguous
 //             4 M^2 x 32 doubles in HBM -> filled by ONE cp.async.bulk (TMA) each, mbarrier-tracked;
 //             the copy for row j+2 is in flight while row j is computed
-//   sN        x-direction part of N for the row in flight ([v][r][q][lane]; transposes ownership
-//             from eta-lines to xi-columns)
+//   sN        first the landing buffer of the row's u^n tile (TMA, issued as soon as the previous
+//             row has let go of it), then a u^n + the x-direction part of beta N
+//             ([v][r][q][lane]; transposes ownership from eta-lines to xi-columns)
 //   sRi       1/sqrt(x^2+y^2+eps^2) at the row's volume nodes (shared by c_s^2 and the star gravity)
-//   sEdge[2]  the two x-neighbour cells outside the block, prefetched one row ahead
+//   sAvg      partial cell averages of the row just written (fused CFL reduction, row a10)
 // ---------------------------------------------------------------------------------------------
 constexpr int NST = 3;
 
 template <int M>
 constexpr size_t stage_smem_bytes() {
-  // tiles + sN + sRi + sEdge + mbarriers
-  return ((size_t)(NST + 1) * 4 * M * M * 32 + (size_t)M * M * 32 + (size_t)4 * 4 * M * M) * sizeof(double) + 64;
+  // tiles + sN + sRi + sAvg + mbarriers
+  return ((size_t)(NST + 1) * 4 * M * M * 32 + (size_t)M * M * 32 + (size_t)4 * M * 32) * sizeof(double) + 64;
 }
 
 template <int M, int EOS, int GRAV, int KIND, int MINB>
@@ -207,19 +209,19 @@ __global__ void __launch_bounds__(M * 32, MINB)
 stage_kernel(const __grid_constant__ StageArgs A) {
   constexpr bool grav = GRAV != G_NONE;
   constexpr bool need_ri = EOS == 1 || grav;
+  constexpr bool add_u = KIND != K_RHS;
   constexpr bool use_un = KIND >= K_MID;
   constexpr bool do_cfl = KIND >= K_LAST;
   constexpr bool do_damp = KIND == K_LASTD;
   constexpr int C = 4 * M * M;                   // doubles per cell
   constexpr int BS = C * 32;                     // doubles per 32-cell tile
-  constexpr int NT = M * 32;
   constexpr uint32_t TILE_BYTES = BS * sizeof(double);
   extern __shared__ __align__(128) double smem[];
   double* tiles = smem;
   double* sN = tiles + NST * BS;
   double* sRi = sN + BS;                         // [r][q][lane]
-  double* sEdge = sRi + M * M * 32;              // [slot][side][C]
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(sEdge + 4 * C);
+  double* sAvg = sRi + M * M * 32;               // [v][q][lane]
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(sAvg + 4 * M * 32);   // [NST] tiles, [NST] u^n
 
   const int tid = threadIdx.x;
   const int lane = tid & 31;
@@ -238,31 +240,17 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   const double xW = g.x0 + i * g.dx, xE = g.x0 + (i + 1) * g.dx;
   const double xq_col = xc + g.hdx * T.xi[w];    // x of this thread's column (Y phase)
 
-  // x-neighbour cells outside this block: (cell index, or -1 when there is none)
+  // x-neighbour cells outside this block: (cell index, or -1 when there is none).  Lanes 0..7 of
+  // warp r fetch line r of those two cells straight from L2 (their own blocks are loading the same
+  // rows at about the same time): lane = side * 4 + v.
   const int iLn = ib > 0 ? ib * 32 - 1 : (g.bc == 0 ? g.nx - 1 : -1);
   const int iRn = ib * 32 + 32 < g.nx ? ib * 32 + 32 : (g.bc == 0 ? 0 : -1);
-  const double* edgeL = iLn >= 0 ? A.qprev + (size_t)(iLn >> 5) * BS + (iLn & 31) : nullptr;
-  const double* edgeR = iRn >= 0 ? A.qprev + (size_t)(iRn >> 5) * BS + (iRn & 31) : nullptr;
-  constexpr int NE = (2 * C + NT - 1) / NT;      // edge elements per thread
-  auto edge_load = [&](int jj, double (&e)[NE]) {
-#pragma unroll
-    for (int k = 0; k < NE; ++k) {
-      const int idx = tid + k * NT;
-      e[k] = 0.0;
-      if (idx < 2 * C) {
-        const double* src = idx < C ? edgeL : edgeR;
-        const int el = idx < C ? idx : idx - C;
-        if (src) e[k] = __ldg(src + (size_t)jj * row_stride + el * 32);
-      }
-    }
-  };
-  auto edge_store = [&](int slot, const double (&e)[NE]) {
-#pragma unroll
-    for (int k = 0; k < NE; ++k) {
-      const int idx = tid + k * NT;
-      if (idx < 2 * C) sEdge[slot * 2 * C + idx] = e[k];
-    }
-  };
+  const bool haveL = iLn >= 0, haveR = iRn >= 0;
+  const double* edge_src = nullptr;
+  if (lane < 8) {
+    const int ic = lane < 4 ? iLn : iRn;
+    if (ic >= 0) edge_src = A.qprev + (size_t)(ic >> 5) * BS + (ic & 31) + (size_t)(((lane & 3) * M + w) * M) * 32;
+  }
 
   // tile t holds row j0-1+t (wrapped for periodic domains; absent outside a non-periodic domain)
   auto tile_row = [&](int t) -> int {
@@ -271,9 +259,9 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     if (jj >= g.ny) return g.bc == 0 ? 0 : -1;
     return jj;
   };
-  auto tile_issue = [&](int t) {
+  auto tile_issue = [&](int t) {                 // thread 0 only
     const int jr = tile_row(t);
-    if (tid == 0 && jr >= 0) {
+    if (jr >= 0) {
       uint64_t* bar = mbar + t % NST;
       mbar_expect_tx(bar, TILE_BYTES);
       bulk_g2s(tiles + (t % NST) * BS, A.qprev + jr * row_stride + (size_t)ib * BS, TILE_BYTES, bar);
@@ -285,23 +273,34 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   auto tile_wait = [&](int t) {
     if (tile_row(t) >= 0) mbar_wait(mbar + t % NST, (uint32_t)((t / NST - (t % NST == 0 ? skip0 : 0)) & 1));
   };
+  auto un_issue = [&](int j) {                   // thread 0 only; u^n tile of row j -> sN
+    mbar_expect_tx(mbar + NST, TILE_BYTES);
+    bulk_g2s(sN, A.qn + (size_t)j * row_stride + (size_t)ib * BS, TILE_BYTES, mbar + NST);
+  };
+  // the last stage also reads the initial state where the wave-killing zone is active: pull that
+  // tile into L2 ahead of its use (cheap test on the tile's farthest corner)
+  auto prefetch_q0 = [&](int j) {                // thread 0 only
+    const double xa = fmax(fabs(g.x0 + ib * 32 * g.dx), fabs(g.x0 + (ib * 32 + 32) * g.dx));
+    const double ya = fmax(fabs(g.y0 + j * g.dy), fabs(g.y0 + (j + 1) * g.dy));
+    if (xa * xa + ya * ya > A.damp_r0 * A.damp_r0)
+      bulk_prefetch_l2(A.q0 + (size_t)j * row_stride + (size_t)ib * BS, TILE_BYTES);
+  };
 
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < NST; ++s) mbar_init(mbar + s, 1);
+    for (int s = 0; s <= NST; ++s) mbar_init(mbar + s, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  tile_issue(0);
-  tile_issue(1);
-  tile_issue(2);
-  {
-    double e[NE];
-    edge_load(j0, e);
-    edge_store(j0 & 1, e);
+  if (tid == 0) {
+    tile_issue(0);
+    tile_issue(1);
+    tile_issue(2);
+    if (use_un) un_issue(j0);
+    if (do_damp) prefetch_q0(j0);
   }
 
-  // numerical flux through the south face of the row about to be processed, column q = w
+  // numerical flux (x2) through the south face of the row about to be processed, column q = w
   double HS[4];
   bool have_HS = false;
   double spmax = 0.0;                            // running CFL wave-speed maximum of this lane (warp 0)
@@ -325,26 +324,28 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     }
     if (have_below) euler_flux<EOS, 1, true>(A.ph, bU, cs2, ciso, bG, bLam);
   }
-  __syncthreads();                               // tile 0's slot may be refilled; sEdge[j0&1] visible
+  __syncthreads();                               // tile 0's slot may be refilled
 
   for (int j = j0; j < j1; ++j) {
     const int t = j - j0 + 1;                    // tile index of row j
-    if (j + 1 < j1) tile_issue(t + 2);           // row j+2 -> the slot row j-1 has just left
+    const bool more = j + 1 < j1;
+    if (tid == 0) {
+      fence_proxy_async();                       // the slots about to be refilled were read through the generic proxy
+      if (more) tile_issue(t + 2);               // row j+2 -> the slot row j-1 has just left
+      if (use_un && j > j0) un_issue(j);         // sN is free again
+      if (do_damp && more) prefetch_q0(j + 1);
+    }
     const double* tu = tiles + (t % NST) * BS + lane;
     const double yc = g.y0 + (j + 0.5) * g.dy;
-    double enext[NE];
-    const bool more = j + 1 < j1;
-    if (more) edge_load(j + 1, enext);
 
-    // fused CFL wave speed of the row finished in the previous iteration (row a10).
-    // Partial cell averages were parked in sN[v][r=0][q][lane], which only this warp rewrites.
+    // fused CFL wave speed of the row finished in the previous iteration (row a10)
     if (do_cfl && w == 0 && j > j0) {
       double avg[4];
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
         double s = 0.0;
 #pragma unroll
-        for (int qq = 0; qq < M; ++qq) s += sN[((v * M + 0) * M + qq) * 32 + lane];
+        for (int qq = 0; qq < M; ++qq) s += sAvg[(v * M + qq) * 32 + lane];
         avg[v] = s;
       }
       double sp = 0.0;
@@ -361,10 +362,13 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       spmax = fmax(spmax, sp);                   // per lane; reduced once after the last row
     }
 
-    tile_wait(t);
     // =========================== X phase: eta-line r = w ===========================
     {
       const int r = w;
+      double eraw[M];                            // lanes 0..7: line r of the two out-of-block neighbours
+#pragma unroll
+      for (int q = 0; q < M; ++q) eraw[q] = edge_src ? __ldg(edge_src + (size_t)j * row_stride + q * 32) : 0.0;
+      tile_wait(t);
       const double yr = yc + g.hdy * T.xi[r];
       const double y2e = fma(yr, yr, A.ph.eps2s);
       double acc[4][M];
@@ -397,6 +401,14 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 #pragma unroll
           for (int qq = 0; qq < M; ++qq) acc[v][qq] = fma(T.Dx[qq][q], F[v], acc[v][qq]);
       }
+      // traces of the two out-of-block neighbours: lane side*4+v reduces its line; lane 0 picks up the
+      // left one (lanes 0..3), the last lane the right one (lanes 4..7)
+      double etr = 0.0;
+#pragma unroll
+      for (int q = 0; q < M; ++q) etr = fma(lane < 4 ? T.Ip[q] : T.Im[q], eraw[q], etr);
+      double UX[4];
+#pragma unroll
+      for (int v = 0; v < 4; ++v) UX[v] = __shfl_sync(FULL, etr, (lane == 0 ? 0 : 4) + v);
       // own W/E face states, fluxes, speeds; c_s at the E face is the right neighbour's W value
       double cs2W = 0.0, cW = 0.0, cs2E = 0.0, cE = 0.0;
       if (EOS == 1) {
@@ -416,26 +428,34 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 #pragma unroll
       for (int v = 0; v < 4; ++v) { UR[v] = shfl_dn1(UW[v]); FR[v] = shfl_dn1(FWo[v]); }
       lamR = shfl_dn1(lamWo);
+      if (last_lane == 0) {                      // a one-cell block: lane 0 needs both neighbours
+#pragma unroll
+        for (int v = 0; v < 4; ++v) UR[v] = __shfl_sync(FULL, etr, 4 + v);
+      } else if (lane == last_lane) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v) UR[v] = UX[v];
+      }
       if (lane == last_lane) {                   // right neighbour is outside this block
-        if (edgeR) {
-          line_trace<M>(sEdge + (j & 1) * 2 * C + C, 1, r, T.Im, UR);
-        } else if (g.bc == 1) {
+        if (!haveR) {
+          if (g.bc == 1) {
 #pragma unroll
-          for (int v = 0; v < 4; ++v) UR[v] = UE[v];
-        } else {
+            for (int v = 0; v < 4; ++v) UR[v] = UE[v];
+          } else {
 #pragma unroll
-          for (int v = 0; v < 4; ++v) UR[v] = __ldg(A.btrE + ((size_t)j * 4 + v) * M + r);
+            for (int v = 0; v < 4; ++v) UR[v] = __ldg(A.btrE + ((size_t)j * 4 + v) * M + r);
+          }
         }
         euler_flux<EOS, 0, true>(A.ph, UR, cs2E, cE, FR, lamR);
       }
       double HE[4], HW[4];
-      llf(UE, FEo, lamEo, UR, FR, lamR, HE);
+      llf2(UE, FEo, lamEo, UR, FR, lamR, HE);
 #pragma unroll
       for (int v = 0; v < 4; ++v) HW[v] = shfl_up1(HE[v]);
       if (lane == 0) {                           // left neighbour is outside this block
         double UL[4], FL[4], lamL;
-        if (edgeL) {
-          line_trace<M>(sEdge + (j & 1) * 2 * C, 1, r, T.Ip, UL);
+        if (haveL) {
+#pragma unroll
+          for (int v = 0; v < 4; ++v) UL[v] = UX[v];
         } else if (g.bc == 1) {
 #pragma unroll
           for (int v = 0; v < 4; ++v) UL[v] = UW[v];
@@ -444,14 +464,19 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           for (int v = 0; v < 4; ++v) UL[v] = __ldg(A.btrW + ((size_t)j * 4 + v) * M + r);
         }
         euler_flux<EOS, 0, true>(A.ph, UL, cs2W, cW, FL, lamL);
-        llf(UL, FL, lamL, UW, FWo, lamWo, HW);
+        llf2(UL, FL, lamL, UW, FWo, lamWo, HW);
       }
+      // a u^n (landed in sN) + x-part of beta N
+      if (use_un) mbar_wait(mbar + NST, (uint32_t)((t - 1) & 1));
 #pragma unroll
       for (int v = 0; v < 4; ++v)
 #pragma unroll
-        for (int qq = 0; qq < M; ++qq)
-          sN[((v * M + r) * M + qq) * 32 + lane] =
-              fma(T.lxm[qq], HW[v], fma(-T.lxp[qq], HE[v], acc[v][qq]));
+        for (int qq = 0; qq < M; ++qq) {
+          double* p = sN + ((v * M + r) * M + qq) * 32 + lane;
+          double val = fma(T.lxm[qq], HW[v], fma(-T.lxp[qq], HE[v], acc[v][qq]));
+          if (use_un) val = fma(A.a, *p, val);
+          *p = val;
+        }
     }
     __syncthreads();
 
@@ -459,14 +484,6 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     {
       const int q = w;
       const double xq = xq_col;
-      const double* __restrict__ qn = A.qn + j * row_stride + (size_t)ib * BS + lane;
-      double un[4][M];
-      if (use_un) {
-#pragma unroll
-        for (int v = 0; v < 4; ++v)
-#pragma unroll
-          for (int rr = 0; rr < M; ++rr) un[v][rr] = __ldg(qn + ((v * M + rr) * M + q) * 32);
-      }
       double acc[4][M];
 #pragma unroll
       for (int v = 0; v < 4; ++v)
@@ -488,13 +505,13 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           const double ri = sRi[(r * M + q) * 32 + lane];
           if (EOS == 1) cs2 = A.ph.h2gm * ri;
           if (grav) {
-            const double k = -A.ph.gm * ri * ri * ri;
+            const double k = -A.ph.gmb * ri * ri * ri;
             gx = k * xq;
             gy = k * yr;
             if (GRAV == G_PLANET) {
               const double ddx = xq - A.ph.xp, ddy = yr - A.ph.yp;
               const double rpi = rsqrt_fast(fma(ddx, ddx, fma(ddy, ddy, A.ph.eps2p)));
-              const double kp = -A.ph.qgm * rpi * rpi * rpi;
+              const double kp = -A.ph.qgmb * rpi * rpi * rpi;
               gx = fma(kp, ddx, gx);
               gy = fma(kp, ddy, gy);
             }
@@ -510,6 +527,10 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           acc[1][r] = fma(u[0], gx, acc[1][r]);
           acc[2][r] = fma(u[0], gy, acc[2][r]);
           acc[3][r] = fma(u[1], gx, fma(u[2], gy, acc[3][r]));
+        }
+        if (add_u) {                             // + b u^(s-1)  (b = 1 in the first stage)
+#pragma unroll
+          for (int v = 0; v < 4; ++v) acc[v][r] = KIND == K_FIRST ? acc[v][r] + u[v] : fma(A.b, u[v], acc[v][r]);
         }
       }
       // south face: carried from the previous row, or built once at the start of the segment
@@ -529,7 +550,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           for (int v = 0; v < 4; ++v) { bU[v] = US[v]; bG[v] = GSo[v]; }
           bLam = lamSo;
         }
-        llf(bU, bG, bLam, US, GSo, lamSo, HS);
+        llf2(bU, bG, bLam, US, GSo, lamSo, HS);
         have_HS = true;
       }
       // north face: own trace against the S trace of the row above (tile t+1)
@@ -556,7 +577,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
         euler_flux<EOS, 1, true>(A.ph, aU, cs2N, cN, aG, aLam);
       }
       double HN[4];
-      llf(UN, GNo, lamNo, aU, aG, aLam, HN);
+      llf2(UN, GNo, lamNo, aU, aG, aLam, HN);
 
       // wave-killing factors of this cell (row a12): out <- f0 u0 + ft out
       double f0 = 0.0, ft = 1.0;
@@ -584,23 +605,16 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 #pragma unroll
         for (int rr = 0; rr < M; ++rr) {
           const int e = ((v * M + rr) * M + q) * 32;
-          const double n = sN[e + lane] + fma(T.lym[rr], HS[v], fma(-T.lyp[rr], HN[v], acc[v][rr]));
-          double out;
-          if (KIND == K_RHS) {
-            out = n;
-          } else {
-            out = fma(A.dt, n, tu[e]);
-            if (use_un) out = fma(A.a, un[v][rr], A.b * out);
-            if (do_damp && damp) out = fma(f0, __ldg(q0 + e), ft * out);
-          }
+          double out = sN[e + lane] + acc[v][rr];
+          out = fma(T.lym[rr], HS[v], fma(-T.lyp[rr], HN[v], out));
+          if (do_damp && damp) out = fma(f0, __ldg(q0 + e), ft * out);
           if (valid) qo[e] = out;
           if (do_cfl) avg = fma(T.w[rr], out, avg);
         }
-        if (do_cfl) sN[((v * M + 0) * M + q) * 32 + lane] = 0.25 * T.w[q] * avg;
+        if (do_cfl) sAvg[(v * M + q) * 32 + lane] = 0.25 * T.w[q] * avg;
       }
 #pragma unroll
       for (int v = 0; v < 4; ++v) HS[v] = HN[v];   // this row's N face is the next row's S face
-      if (more) edge_store((j + 1) & 1, enext);
     }
     __syncthreads();
   }
@@ -611,7 +625,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     for (int v = 0; v < 4; ++v) {
       double s = 0.0;
 #pragma unroll
-      for (int qq = 0; qq < M; ++qq) s += sN[((v * M + 0) * M + qq) * 32 + lane];
+      for (int qq = 0; qq < M; ++qq) s += sAvg[(v * M + qq) * 32 + lane];
       avg[v] = s;
     }
     double sp = 0.0;
