@@ -68,7 +68,7 @@ def load_ncu_traffic(order: int, n: int):
     path = os.path.join(ROOT, "profiles", "stage_traffic.csv")
     try:
         with open(path) as f:
-            rows = [ln.strip().split(",") for ln in f if ln.strip() and not ln.startswith("#")]
+            rows = [ln.strip().split(";") for ln in f if ln.strip() and not ln.startswith("#")]
         hdr, rows = rows[0], rows[1:]
         idx = {k: i for i, k in enumerate(hdr)}
         vals = [float(r[idx["dram_read_bytes"]]) + float(r[idx["dram_write_bytes"]]) for r in rows
