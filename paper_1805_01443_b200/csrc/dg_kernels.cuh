@@ -166,14 +166,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       "DONE_%=:\n"
       "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {   // release.cta
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ int atom_add_acq_rel(int* p, int v) {
-  int old;
-  asm volatile("atom.acq_rel.cta.shared::cta.add.s32 %0, [%1], %2;" : "=r"(old) : "r"(smem_u32(p)), "r"(v) : "memory");
-  return old;
-}
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
@@ -201,23 +193,15 @@ __device__ __forceinline__ void fence_proxy_async() {
 //   sN        first the landing buffer of the row's u^n tile (TMA, issued as soon as the previous
 //             row has let go of it), then a u^n + the x-direction part of beta N
 //             ([v][r][q][lane]; transposes ownership from eta-lines to xi-columns)
+//   sRi       1/sqrt(x^2+y^2+eps^2) at the row's volume nodes (shared by c_s^2 and the star gravity)
 //   sAvg      partial cell averages of the row just written (fused CFL reduction, row a10)
-//
-// Synchronisation inside the row loop is split-phase (no __syncthreads): a warp only ever waits for
-// something the other warps produced a whole phase earlier.
-//   x_done    mbarrier, M arrivals: every warp has written its eta-line of sN for this row; waited
-//             for just before the Y-phase epilogue (the Y node loop does not touch sN)
-//   row_done  every warp is through with the row (its tile, sN, sAvg).  The LAST warp to get there
-//             (elected by a shared counter, acq_rel) refills the ring slot and sN by TMA and does the
-//             row's CFL wave speed; nobody blocks.  Stages that do not land u^n in sN wait on the
-//             mbarrier twin of the counter before overwriting sN one X phase later.
 // ---------------------------------------------------------------------------------------------
 constexpr int NST = 3;
 
 template <int M>
 constexpr size_t stage_smem_bytes() {
-  // tiles + sN + sAvg + mbarriers and the row counter
-  return ((size_t)(NST + 1) * 4 * M * M * 32 + (size_t)4 * M * 32) * sizeof(double) + 128;
+  // tiles + sN + sRi + sAvg + mbarriers
+  return ((size_t)(NST + 1) * 4 * M * M * 32 + (size_t)M * M * 32 + (size_t)4 * M * 32) * sizeof(double) + 64;
 }
 
 template <int M, int EOS, int GRAV, int KIND, int MINB>
@@ -235,11 +219,9 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   extern __shared__ __align__(128) double smem[];
   double* tiles = smem;
   double* sN = tiles + NST * BS;
-  double* sAvg = sN + BS;                        // [v][q][lane]
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(sAvg + 4 * M * 32);   // [NST] tiles, u^n, x_done, row_done
-  uint64_t* bar_x = mbar + NST + 1;
-  uint64_t* bar_row = mbar + NST + 2;
-  int* row_cnt = reinterpret_cast<int*>(mbar + NST + 3);
+  double* sRi = sN + BS;                         // [r][q][lane]
+  double* sAvg = sRi + M * M * 32;               // [v][q][lane]
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(sAvg + 4 * M * 32);   // [NST] tiles, [NST] u^n
 
   const int tid = threadIdx.x;
   const int lane = tid & 31;
@@ -307,9 +289,6 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s <= NST; ++s) mbar_init(mbar + s, 1);
-    mbar_init(bar_x, M);
-    mbar_init(bar_row, M);
-    *row_cnt = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -318,61 +297,89 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     tile_issue(1);
     tile_issue(2);
     if (use_un) un_issue(j0);
-    if (do_damp) {
-      prefetch_q0(j0);
-      if (j0 + 1 < j1) prefetch_q0(j0 + 1);
-    }
+    if (do_damp) prefetch_q0(j0);
   }
+
   // line r = w of the two out-of-block x-neighbours, fetched one row ahead (lanes 0..7)
   double eraw[M];
 #pragma unroll
   for (int q = 0; q < M; ++q) eraw[q] = edge_src ? __ldg(edge_src + (size_t)j0 * row_stride + q * 32) : 0.0;
 
-  // numerical flux (x2) through the south face of the row about to be processed, column q = w
+  // numerical flux (x2) through the south face of the segment's first row, column q = w: the only
+  // face whose two sides are both evaluated here; afterwards a row's N flux is the next row's S flux
   double HS[4];
-  bool have_HS = false;
-  double spmax = 0.0;                            // running CFL wave-speed maximum of this lane
-  double bU[4], bG[4], bLam = 0.0;               // north-face data of the row below (first row only)
-  bool have_below = false;
-  const double x2e_col = fma(xq_col, xq_col, A.ph.eps2s);
+  double spmax = 0.0;                            // running CFL wave-speed maximum of this lane (warp 0)
   {
-    tile_wait(0);
     const double yS = g.y0 + j0 * g.dy;
     double cs2 = 0.0, ciso = 0.0;
     if (EOS == 1) {
-      cs2 = A.ph.h2gm * rsqrt_fast(fma(yS, yS, x2e_col));
+      cs2 = A.ph.h2gm * rsqrt_fast(fma(xq_col, xq_col, fma(yS, yS, A.ph.eps2s)));
       ciso = sqrt_fast(cs2);
     }
+    double US[4], GSo[4], lamSo, bU[4], bG[4], bLam;
+    tile_wait(1);
+    column_trace<M>(tiles + BS + lane, 32, w, T.Im, US);
+    euler_flux<EOS, 1, true>(A.ph, US, cs2, ciso, GSo, lamSo);
     if (tile_row(0) >= 0) {
+      tile_wait(0);
       column_trace<M>(tiles + lane, 32, w, T.Ip, bU);
-      have_below = true;
+      euler_flux<EOS, 1, true>(A.ph, bU, cs2, ciso, bG, bLam);
     } else if (g.bc == 2) {
 #pragma unroll
       for (int v = 0; v < 4; ++v) bU[v] = __ldg(A.btrS + ((size_t)(ib * 4 + v) * M + w) * 32 + lane);
-      have_below = true;
+      euler_flux<EOS, 1, true>(A.ph, bU, cs2, ciso, bG, bLam);
+    } else {                                     // transmissive bottom boundary
+#pragma unroll
+      for (int v = 0; v < 4; ++v) { bU[v] = US[v]; bG[v] = GSo[v]; }
+      bLam = lamSo;
     }
-    if (have_below) euler_flux<EOS, 1, true>(A.ph, bU, cs2, ciso, bG, bLam);
+    llf2(bU, bG, bLam, US, GSo, lamSo, HS);
   }
   __syncthreads();                               // tile 0's slot may be refilled
-  if (tid == 0 && j0 + 1 < j1) {
-    fence_proxy_async();                         // the slot was read through the generic proxy
-    tile_issue(3);                               // row j0+2
-  }
 
   for (int j = j0; j < j1; ++j) {
     const int t = j - j0 + 1;                    // tile index of row j
     const bool more = j + 1 < j1;
-    const uint32_t rpar = (uint32_t)((j - j0) & 1);
+    if (tid == 0) {
+      fence_proxy_async();                       // the slots about to be refilled were read through the generic proxy
+      if (more) tile_issue(t + 2);               // row j+2 -> the slot row j-1 has just left
+      if (use_un && j > j0) un_issue(j);         // sN is free again
+      if (do_damp && more) prefetch_q0(j + 1);
+    }
     const double* tu = tiles + (t % NST) * BS + lane;
     const double yc = g.y0 + (j + 0.5) * g.dy;
-    double enext[M];
+
+    // fused CFL wave speed of the row finished in the previous iteration (row a10)
+    if (do_cfl && w == 0 && j > j0) {
+      double avg[4];
 #pragma unroll
-    for (int q = 0; q < M; ++q)
-      enext[q] = (more && edge_src) ? __ldg(edge_src + (size_t)(j + 1) * row_stride + q * 32) : 0.0;
+      for (int v = 0; v < 4; ++v) {
+        double s = 0.0;
+#pragma unroll
+        for (int qq = 0; qq < M; ++qq) s += sAvg[(v * M + qq) * 32 + lane];
+        avg[v] = s;
+      }
+      double sp = 0.0;
+      if (valid) {
+        const double ycp = g.y0 + (j - 0.5) * g.dy;
+        const double rinv = 1.0 / avg[0];
+        const double vx = avg[1] * rinv, vy = avg[2] * rinv;
+        double c;
+        if (EOS == 0) c = sqrt(A.ph.gamma * A.ph.gm1 * (avg[3] - 0.5 * (avg[1] * vx + avg[2] * vy)) * rinv);
+        else          c = sqrt(A.ph.h2gm * rsqrt(fma(xc, xc, fma(ycp, ycp, A.ph.eps2s))));
+        sp = (fabs(vx) + c) * g.inv_dx + (fabs(vy) + c) * g.inv_dy;
+        if (!(sp >= 0.0)) sp = __longlong_as_double(0x7ff0000000000000LL);   // NaN -> +inf
+      }
+      spmax = fmax(spmax, sp);                   // per lane; reduced once after the last row
+    }
 
     // =========================== X phase: eta-line r = w ===========================
     {
       const int r = w;
+      double enext[M];                           // next row's edge lines: in flight during this row
+#pragma unroll
+      for (int q = 0; q < M; ++q)
+        enext[q] = (edge_src && more) ? __ldg(edge_src + (size_t)(j + 1) * row_stride + q * 32) : 0.0;
       tile_wait(t);
       const double yr = yc + g.hdy * T.xi[r];
       const double y2e = fma(yr, yr, A.ph.eps2s);
@@ -393,9 +400,11 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           UE[v] = fma(T.Ip[q], u[v], UE[v]);
         }
         double cs2 = 0.0;
-        if (EOS == 1) {
+        if (need_ri) {
           const double xq = xc + g.hdx * T.xi[q];
-          cs2 = A.ph.h2gm * rsqrt_fast(fma(xq, xq, y2e));
+          const double ri = rsqrt_fast(fma(xq, xq, y2e));
+          sRi[(r * M + q) * 32 + lane] = ri;
+          if (EOS == 1) cs2 = A.ph.h2gm * ri;
         }
         double F[4], dummy;
         euler_flux<EOS, 0, false>(A.ph, u, cs2, 0.0, F, dummy);
@@ -409,6 +418,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       double etr = 0.0;
 #pragma unroll
       for (int q = 0; q < M; ++q) etr = fma(lane < 4 ? T.Ip[q] : T.Im[q], eraw[q], etr);
+#pragma unroll
+      for (int q = 0; q < M; ++q) eraw[q] = enext[q];
       double UX[4];
 #pragma unroll
       for (int v = 0; v < 4; ++v) UX[v] = __shfl_sync(FULL, etr, (lane == 0 ? 0 : 4) + v);
@@ -469,10 +480,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
         euler_flux<EOS, 0, true>(A.ph, UL, cs2W, cW, FL, lamL);
         llf2(UL, FL, lamL, UW, FWo, lamWo, HW);
       }
-      // a u^n (landed in sN) + x-part of beta N.  sN is free once every warp is through with the
-      // previous row: implied by the u^n copy having been issued, else waited for explicitly.
-      if (use_un) mbar_wait(mbar + NST, rpar);
-      else if (j > j0) mbar_wait(bar_row, rpar ^ 1u);
+      // a u^n (landed in sN) + x-part of beta N
+      if (use_un) mbar_wait(mbar + NST, (uint32_t)((t - 1) & 1));
 #pragma unroll
       for (int v = 0; v < 4; ++v)
 #pragma unroll
@@ -482,11 +491,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           if (use_un) val = fma(A.a, *p, val);
           *p = val;
         }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar_x);
-#pragma unroll
-      for (int q = 0; q < M; ++q) eraw[q] = enext[q];
     }
+    __syncthreads();
 
     // =========================== Y phase: xi-column q = w ===========================
     {
@@ -498,7 +504,6 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 #pragma unroll
         for (int r = 0; r < M; ++r) acc[v][r] = 0.0;
       double UN[4] = {0, 0, 0, 0};
-      const bool first = !have_HS;
 #pragma unroll
       for (int r = 0; r < M; ++r) {
         double u[4];
@@ -510,7 +515,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
         double cs2 = 0.0, gx = 0.0, gy = 0.0;
         if (need_ri) {
           const double yr = yc + g.hdy * T.xi[r];
-          const double ri = rsqrt_fast(fma(yr, yr, x2e_col));
+          const double ri = sRi[(r * M + q) * 32 + lane];
           if (EOS == 1) cs2 = A.ph.h2gm * ri;
           if (grav) {
             const double k = -A.ph.gmb * ri * ri * ri;
@@ -541,31 +546,11 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           for (int v = 0; v < 4; ++v) acc[v][r] = KIND == K_FIRST ? acc[v][r] + u[v] : fma(A.b, u[v], acc[v][r]);
         }
       }
-      // south face: carried from the previous row, or built once at the start of the segment
-      if (first) {
-        double US[4];
-        column_trace<M>(tu, 32, q, T.Im, US);
-        const double yS = g.y0 + j * g.dy;
-        double cs2 = 0.0, ciso = 0.0;
-        if (EOS == 1) {
-          cs2 = A.ph.h2gm * rsqrt_fast(fma(yS, yS, x2e_col));
-          ciso = sqrt_fast(cs2);
-        }
-        double GSo[4], lamSo;
-        euler_flux<EOS, 1, true>(A.ph, US, cs2, ciso, GSo, lamSo);
-        if (!have_below) {                       // transmissive bottom boundary
-#pragma unroll
-          for (int v = 0; v < 4; ++v) { bU[v] = US[v]; bG[v] = GSo[v]; }
-          bLam = lamSo;
-        }
-        llf2(bU, bG, bLam, US, GSo, lamSo, HS);
-        have_HS = true;
-      }
       // north face: own trace against the S trace of the row above (tile t+1)
       const double yN = g.y0 + (j + 1) * g.dy;
       double cs2N = 0.0, cN = 0.0;
       if (EOS == 1) {
-        cs2N = A.ph.h2gm * rsqrt_fast(fma(yN, yN, x2e_col));
+        cs2N = A.ph.h2gm * rsqrt_fast(fma(xq, xq, fma(yN, yN, A.ph.eps2s)));
         cN = sqrt_fast(cs2N);
       }
       double GNo[4], lamNo;
@@ -607,7 +592,6 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       // modal update in nodal form + RK combination (rows a8, a9) and store
       double* __restrict__ qo = A.qout + j * row_stride + (size_t)ib * BS + lane;
       const double* __restrict__ q0 = A.q0 + j * row_stride + (size_t)ib * BS + lane;
-      mbar_wait(bar_x, rpar);                    // every eta-line of sN has been written
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
         double avg = 0.0;
@@ -625,54 +609,37 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 #pragma unroll
       for (int v = 0; v < 4; ++v) HS[v] = HN[v];   // this row's N face is the next row's S face
     }
-
-    // ---- this warp is through with row j; the last warp out refills the buffers and does the CFL
-    __syncwarp();
-    int order = 0;
-    if (lane == 0) {
-      if (!use_un) mbar_arrive(bar_row);
-      order = atom_add_acq_rel(row_cnt, 1);
-    }
-    order = __shfl_sync(FULL, order, 0);
-    if (order == M * (j - j0 + 1) - 1) {
-      if (lane == 0) {
-        fence_proxy_async();                     // the buffers were read through the generic proxy
-        if (j + 2 < j1) tile_issue(t + 3);       // row j+3 -> the slot row j has just left
-        if (use_un && more) un_issue(j + 1);     // sN is free again
-        if (do_damp && j + 2 < j1) prefetch_q0(j + 2);
-      }
-      if (do_cfl) {                              // fused CFL wave speed of row j (row a10)
-        double avg[4];
-#pragma unroll
-        for (int v = 0; v < 4; ++v) {
-          double s = 0.0;
-#pragma unroll
-          for (int qq = 0; qq < M; ++qq) s += sAvg[(v * M + qq) * 32 + lane];
-          avg[v] = s;
-        }
-        double sp = 0.0;
-        if (valid) {
-          const double rinv = 1.0 / avg[0];
-          const double vx = avg[1] * rinv, vy = avg[2] * rinv;
-          double c;
-          if (EOS == 0) c = sqrt(A.ph.gamma * A.ph.gm1 * (avg[3] - 0.5 * (avg[1] * vx + avg[2] * vy)) * rinv);
-          else          c = sqrt(A.ph.h2gm * rsqrt(fma(xc, xc, fma(yc, yc, A.ph.eps2s))));
-          sp = (fabs(vx) + c) * g.inv_dx + (fabs(vy) + c) * g.inv_dy;
-          if (!(sp >= 0.0)) sp = __longlong_as_double(0x7ff0000000000000LL);   // NaN -> +inf
-        }
-        spmax = fmax(spmax, sp);                 // per lane of whichever warp was last; reduced below
-      }
-    }
+    __syncthreads();
   }
-  if (do_cfl) {
+  // CFL wave speed of the last row of the segment, then one reduction per thread block
+  if (do_cfl && w == 0) {
+    double avg[4];
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+      double s = 0.0;
+#pragma unroll
+      for (int qq = 0; qq < M; ++qq) s += sAvg[(v * M + qq) * 32 + lane];
+      avg[v] = s;
+    }
+    double sp = 0.0;
+    if (valid) {
+      const double ycp = g.y0 + (j1 - 0.5) * g.dy;
+      const double rinv = 1.0 / avg[0];
+      const double vx = avg[1] * rinv, vy = avg[2] * rinv;
+      double c;
+      if (EOS == 0) c = sqrt(A.ph.gamma * A.ph.gm1 * (avg[3] - 0.5 * (avg[1] * vx + avg[2] * vy)) * rinv);
+      else          c = sqrt(A.ph.h2gm * rsqrt(fma(xc, xc, fma(ycp, ycp, A.ph.eps2s))));
+      sp = (fabs(vx) + c) * g.inv_dx + (fabs(vy) + c) * g.inv_dy;
+      if (!(sp >= 0.0)) sp = __longlong_as_double(0x7ff0000000000000LL);
+    }
     // non-negative doubles order like their bit patterns
-    unsigned long long bits = (unsigned long long)__double_as_longlong(spmax);
+    unsigned long long bits = (unsigned long long)__double_as_longlong(fmax(spmax, sp));
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       const unsigned long long other = __shfl_xor_sync(FULL, bits, o);
       bits = other > bits ? other : bits;
     }
-    if (lane == 0 && bits != 0ull) atomicMax(A.wmax, bits);
+    if (lane == 0) atomicMax(A.wmax, bits);
   }
 }
 
