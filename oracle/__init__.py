@@ -42,6 +42,7 @@ class RefParams(C.Structure):
         ("q_planet", C.c_double), ("r_planet", C.c_double), ("eps_planet", C.c_double),
         ("omega_planet", C.c_double), ("phase0", C.c_double),
         ("damp_r0", C.c_double), ("damp_r1", C.c_double), ("t0", C.c_double),
+        ("limiter", C.c_int32), ("lim_eps", C.c_double),
     ]
 
 
@@ -78,6 +79,8 @@ def _lib(omp: bool):
         "ref_rhs_parts": (i, [vp, d, i, _PD]), "ref_damp": (i, [vp, d]),
         "ref_rk_step": (i, [i, C.c_long, _PD, d, d, _ODE_FN, vp, _PD]),
         "ref_threads": (i, []), "ref_set_threads": (None, [i]),
+        "ref_rk_stages": (i, [i]), "ref_limit": (i, [vp]), "ref_torque": (i, [vp, d, _PD]),
+        "ref_lobatto": (i, [i, _PD, _PD]), "ref_limit_cell": (i, [PP, _PD, _PD]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -148,9 +151,17 @@ class RefDG:
         _chk(self.L.ref_step(self._h, float(dt)), "ref_step")
 
     def step_debug(self, dt: float) -> np.ndarray:
-        st = np.empty((self.params["rk"],) + self.shape)
+        st = np.empty((rk_stages(self.params["rk"]),) + self.shape)
         _chk(self.L.ref_step_debug(self._h, float(dt), _p(st)), "ref_step_debug")
         return st
+
+    def limit(self):
+        _chk(self.L.ref_limit(self._h), "ref_limit")
+
+    def torque(self, t: float) -> float:
+        g = C.c_double()
+        _chk(self.L.ref_torque(self._h, float(t), C.byref(g)), "ref_torque")
+        return g.value
 
     def damp(self, dt: float):
         _chk(self.L.ref_damp(self._h, float(dt)), "ref_damp")
@@ -165,6 +176,28 @@ class RefDG:
 
 
 # ---- pieces, for the pin tests ----------------------------------------------------------------
+def rk_stages(rk: int) -> int:
+    """Sub-steps per time step: 2, 3, 5 (rk 4: SSP-RK(5,4)), 6 (rk 5: Cash-Karp)."""
+    return int(_lib(False).ref_rk_stages(int(rk)))
+
+
+def lobatto(m: int):
+    """Gauss-Lobatto nodes on [-1,1] and weights normalised to sum 1 used by the limiter of order m."""
+    xh, wh = np.empty(4), np.empty(4)
+    n = _lib(False).ref_lobatto(int(m), _p(xh), _p(wh))
+    if n < 0:
+        raise RuntimeError("oracle: ref_lobatto failed")
+    return xh[:n].copy(), wh[:n].copy()
+
+
+def limit_cell(params: dict, u: np.ndarray):
+    """C12 on one cell u[4][m][m]; returns (limited copy, theta1, theta2)."""
+    u = np.array(u, dtype=np.float64).copy()
+    th = np.empty(2)
+    _chk(_lib(False).ref_limit_cell(C.byref(_to_struct(params)), _p(u), _p(th)), "ref_limit_cell")
+    return u, float(th[0]), float(th[1])
+
+
 def tables(m: int) -> dict:
     L = _lib(False)
     xi, w, Ep, Em = (np.empty(m) for _ in range(4))
@@ -209,7 +242,7 @@ def rk_step(rk: int, y: np.ndarray, t: float, dt: float, f, want_stages: bool = 
         yy = np.ctypeslib.as_array(yp, shape=(n,))
         np.ctypeslib.as_array(dp, shape=(n,))[:] = f(tt, yy.copy())
 
-    st = np.empty((rk, n)) if want_stages else None
+    st = np.empty((rk_stages(rk), n)) if want_stages else None
     _chk(L.ref_rk_step(rk, n, _p(y), t, dt, _ODE_FN(cb), None,
                        _p(st) if want_stages else None), "ref_rk_step")
     return (y, st) if want_stages else y

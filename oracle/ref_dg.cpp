@@ -12,6 +12,9 @@
  *   C9  boundaries
  *   C10 CFL
  *   C11 wave damping
+ *   C8b Butcher-form RK PAPER.md:445-457 (Appendix A), Table 1, Table 2
+ *   C12 positivity limiter  PAPER.md:129-131, 150 (Zhang & Shu 2010; readings L1..L5 in DESIGN.md)
+ *   C13 torque on the planet  PAPER.md:321-328  Eq.(6)
  *
  * No blocking, fusion, sum-factorisation or reordering: every sum is written as the nested loop
  * the formula states, in fp64, compiled with -O2 -ffp-contract=off.
@@ -27,6 +30,12 @@
  *   C8  y' = lambda y observed order 2 / 3; exact on polynomials of degree <= order
  *   C7+C8  isentropic-vortex L1 error slope ~ p+1
  *   C10 hand value on a constant state;  C11 R = 0 identity, fixed point, tau -> 0 limit
+ *   C8b the tableaus against the paper's printed digits (tests/golden/rk_tableaus.txt), row sums = c,
+ *       order conditions, observed order 4 / 5 on y' = lambda y and on a non-autonomous ODE
+ *   C12 Gauss-Lobatto closed forms and exactness; the cell average as a convex combination of the
+ *       limiter's point values; averages kept bitwise; admissibility after limiting; identity on
+ *       admissible cells; hand-worked theta on a linear cell; p = eps at the binding point
+ *   C13 torque of a single massive cell by hand; zero for an axisymmetric ring; antisymmetry
  *   absolute per-step values: PARITY UNPINNED (paper prints none).
  */
 #include "ref_dg.h"
@@ -157,11 +166,19 @@ void gravity(const ref_params& p, double t, double x, double y, double* g) {
   }
 }
 
+/* C12 tables (see build_lobatto) */
+struct LimTables {
+  int nh;
+  double xh[4], wh[4];                    /* Lobatto nodes on [-1,1]; weights normalised to sum 1 */
+  double Bh[4][MAXM];                     /* phi_a(xh_k) */
+};
+
 }  // namespace
 
 struct ref_ctx {
   ref_params p;
   Tables T;
+  LimTables LT;
   int m;
   long ncoef;                 /* ny*nx*4*m*m */
   double dx, dy, t;
@@ -345,15 +362,198 @@ void damp(ref_ctx* c, double dt) {
     }
 }
 
+/* ---- C12: positivity-preserving limiter (Zhang & Shu 2010, step (iii)(d) PAPER.md:150) ----
+ * Point set S_K of a rectangle (Zhang & Shu 2010, their S_ij): (Gauss_m in x) x (Lobatto_nh in y) united
+ * with (Lobatto_nh in x) x (Gauss_m in y), nh the smallest Gauss-Lobatto rule exact for degree
+ * N_p: 2 nh - 3 >= N_p. */
+
+void build_lobatto(int m, LimTables* LT) {
+  const int Np = m - 1;
+  int nh = 2;
+  while (2 * nh - 3 < Np) ++nh;
+  LT->nh = nh;
+  const int n = nh - 1;                   /* interior nodes are the roots of P_n' */
+  const double pi = 3.14159265358979323846;
+  LT->xh[0] = -1.0; LT->xh[n] = 1.0;
+  for (int k = 1; k < n; ++k) {
+    double x = -std::cos(pi * k / n);     /* Chebyshev-Lobatto guess, ascending */
+    for (int it = 0; it < 100; ++it) {
+      double P, dP;
+      legendre(n, x, &P, &dP);
+      const double d2P = (2.0 * x * dP - n * (n + 1.0) * P) / (1.0 - x * x);   /* Legendre's equation */
+      const double dx = dP / d2P;
+      x -= dx;
+      if (std::fabs(dx) < 1e-16) break;
+    }
+    LT->xh[k] = x;
+  }
+  if (n % 2 == 0) LT->xh[n / 2] = 0.0;
+  for (int k = 0; k <= n; ++k) {
+    double P, dP;
+    legendre(n, LT->xh[k], &P, &dP);
+    LT->wh[k] = 0.5 * 2.0 / (n * (n + 1.0) * P * P);                          /* sum = 1 */
+    for (int a = 0; a < m; ++a) {
+      double Pa, dPa;
+      legendre(a, LT->xh[k], &Pa, &dPa);
+      LT->Bh[k][a] = std::sqrt(2.0 * a + 1.0) * Pa;
+    }
+  }
+}
+
+/* value of the cell polynomial with basis values px[a] = phi_a(x), py[b] = phi_b(y) */
+void eval_cell(int m, const double* u, const double* px, const double* py, double* out) {
+  for (int v = 0; v < NV; ++v) {
+    double s = 0.0;
+    for (int b = 0; b < m; ++b)
+      for (int a = 0; a < m; ++a) s += u[(v * m + b) * m + a] * px[a] * py[b];
+    out[v] = s;
+  }
+}
+
+inline double pressure_ideal(const ref_params& p, const double* U) {
+  return (p.gamma - 1.0) * (U[3] - 0.5 * (U[1] * U[1] + U[2] * U[2]) / U[0]);
+}
+
+/* the points of S_K, one after the other: k-th point's basis values */
+struct LimPoint { const double* px; const double* py; };
+int limiter_points(const Tables& T, const LimTables& LT, LimPoint* pts) {
+  int n = 0;
+  for (int q = 0; q < T.m; ++q)
+    for (int k = 0; k < LT.nh; ++k) {
+      pts[n].px = T.B[q];  pts[n].py = LT.Bh[k]; ++n;      /* Gauss in x, Lobatto in y */
+      pts[n].px = LT.Bh[k]; pts[n].py = T.B[q];  ++n;      /* Lobatto in x, Gauss in y */
+    }
+  return n;
+}
+
+void limit_cell(const ref_params& p, const Tables& T, const LimTables& LT, double* u, double* theta) {
+  const int m = T.m;
+  double th1 = 1.0, th2 = 1.0;
+  if (m > 1) {
+    LimPoint pts[2 * MAXM * 4];
+    const int npts = limiter_points(T, LT, pts);
+    double ubar[NV];
+    for (int v = 0; v < NV; ++v) ubar[v] = u[v * m * m];          /* mode (0,0) = cell average */
+    /* step 1: density.  theta1 = min(1, (rhobar - eps)/(rhobar - rho_min)) */
+    double rho_min = ubar[0];
+    for (int k = 0; k < npts; ++k) {
+      double s[NV];
+      eval_cell(m, u, pts[k].px, pts[k].py, s);
+      if (s[0] < rho_min) rho_min = s[0];
+    }
+    const double eps_rho = std::fmin(p.lim_eps, ubar[0]);
+    if (rho_min < eps_rho) {
+      th1 = (ubar[0] - eps_rho) / (ubar[0] - rho_min);
+      for (int k = 1; k < m * m; ++k) u[k] *= th1;                /* rho <- rhobar + theta1 (rho - rhobar) */
+    }
+    /* step 2: pressure (ideal gas only; the isothermal closure has p = c_s^2 rho > 0 with rho).
+     * For every point with p < eps, the intersection s(t) = ubar + t (u(x) - ubar) of the segment
+     * with the surface p = eps; theta2 = min t. */
+    if (p.eos == 0) {
+      const double pbar = pressure_ideal(p, ubar);
+      const double eps_p = std::fmin(p.lim_eps, pbar);
+      const double e1 = eps_p / (p.gamma - 1.0);
+      for (int k = 0; k < npts; ++k) {
+        double s[NV];
+        eval_cell(m, u, pts[k].px, pts[k].py, s);
+        if (pressure_ideal(p, s) < eps_p) {
+          /* g(t) = E(t) rho(t) - |m(t)|^2/2 - e1 rho(t) = A t^2 + B t + C, g(0) >= 0 > g(1) */
+          const double dr = s[0] - ubar[0], dmx = s[1] - ubar[1], dmy = s[2] - ubar[2], dE = s[3] - ubar[3];
+          const double A = dE * dr - 0.5 * (dmx * dmx + dmy * dmy);
+          const double B = ubar[3] * dr + ubar[0] * dE - (ubar[1] * dmx + ubar[2] * dmy) - e1 * dr;
+          const double C = ubar[3] * ubar[0] - 0.5 * (ubar[1] * ubar[1] + ubar[2] * ubar[2]) - e1 * ubar[0];
+          const double disc = B * B - 4.0 * A * C;
+          const double den = std::sqrt(disc > 0.0 ? disc : 0.0) - B;
+          double t = den > 0.0 ? 2.0 * C / den : 0.0;             /* the root the segment meets first */
+          if (!(t >= 0.0)) t = 0.0;
+          if (t > 1.0) t = 1.0;
+          if (t < th2) th2 = t;
+        }
+      }
+      if (th2 < 1.0)
+        for (int v = 0; v < NV; ++v)
+          for (int k = 1; k < m * m; ++k) u[v * m * m + k] *= th2;
+    }
+  }
+  if (theta) { theta[0] = th1; theta[1] = th2; }
+}
+
+void limit_all(const ref_ctx* c, const LimTables& LT, double* U) {
+#pragma omp parallel for schedule(static)
+  for (int j = 0; j < c->p.ny; ++j)
+    for (int i = 0; i < c->p.nx; ++i) limit_cell(c->p, c->T, LT, U + cell_off(c, i, j), nullptr);
+}
+
+/* ---- C8b: explicit Runge-Kutta in Butcher form (Appendix A) ----
+ * Coefficients typed from the paper: Table 1 and Table 2.
+ * Table 1's printed b row sums to 1 - 8.8e-11 (14 printed digits): b is divided by its sum
+ * (reading G20) so that the scheme stays exactly consistent. */
+struct Butcher { int s; double a[6][6], b[6], c[6]; };
+
+void butcher_tableau(int rk, Butcher* T) {
+  std::memset(T, 0, sizeof *T);
+  if (rk == 4) {
+    T->s = 5;
+    T->c[1] = 0.39175222700392; T->a[1][0] = 0.39175222700392;
+    T->c[2] = 0.58607968896779; T->a[2][0] = 0.21766909633821; T->a[2][1] = 0.36841059262959;
+    T->c[3] = 0.47454236302687; T->a[3][0] = 0.08269208670950; T->a[3][1] = 0.13995850206999;
+    T->a[3][2] = 0.25189177424738;
+    T->c[4] = 0.93501063100924; T->a[4][0] = 0.06796628370320; T->a[4][1] = 0.11503469844438;
+    T->a[4][2] = 0.20703489864929; T->a[4][3] = 0.54497475021237;
+    T->b[0] = 0.14681187618661; T->b[1] = 0.24848290924556; T->b[2] = 0.10425883036650;
+    T->b[3] = 0.27443890091960; T->b[4] = 0.22600748319395;
+    double sum = 0.0;
+    for (int i = 0; i < 5; ++i) sum += T->b[i];
+    for (int i = 0; i < 5; ++i) T->b[i] /= sum;
+  } else {                                /* rk == 5: Cash & Karp 1990 */
+    T->s = 6;
+    T->c[1] = 1.0 / 5.0;  T->a[1][0] = 1.0 / 5.0;
+    T->c[2] = 3.0 / 10.0; T->a[2][0] = 3.0 / 40.0; T->a[2][1] = 9.0 / 40.0;
+    T->c[3] = 3.0 / 5.0;  T->a[3][0] = 3.0 / 10.0; T->a[3][1] = -9.0 / 10.0; T->a[3][2] = 6.0 / 5.0;
+    T->c[4] = 1.0;        T->a[4][0] = -11.0 / 54.0; T->a[4][1] = 5.0 / 2.0; T->a[4][2] = -70.0 / 27.0;
+    T->a[4][3] = 35.0 / 27.0;
+    T->c[5] = 7.0 / 8.0;  T->a[5][0] = 1631.0 / 55296.0; T->a[5][1] = 175.0 / 512.0;
+    T->a[5][2] = 575.0 / 13824.0; T->a[5][3] = 44275.0 / 110592.0; T->a[5][4] = 253.0 / 4096.0;
+    T->b[0] = 37.0 / 378.0; T->b[2] = 250.0 / 621.0; T->b[3] = 125.0 / 594.0; T->b[5] = 512.0 / 1771.0;
+  }
+}
+
+typedef void (*post_fn)(void* user, double* y);   /* applied to every sub-step's result (the limiter) */
+
+/* y_i = y^n + h sum_{j<i} a_ij k_j,  k_i = f(t^n + c_i h, y_i),  y^{n+1} = y^n + h sum_i b_i k_i.
+ * stages receives y_2 .. y_s and y^{n+1}: the results of the s sub-steps. */
+int butcher_step(int rk, long n, double* y, double t, double dt, ref_ode_fn f, void* user,
+                 double* stages, post_fn post, void* post_user) {
+  Butcher T;
+  butcher_tableau(rk, &T);
+  std::vector<std::vector<double>> k(T.s, std::vector<double>(n));
+  std::vector<double> yi(y, y + n);
+  for (int i = 0; i < T.s; ++i) {
+    f(user, t + T.c[i] * dt, yi.data(), k[i].data());
+    const double* coef = (i + 1 < T.s) ? T.a[i + 1] : T.b;
+    for (long e = 0; e < n; ++e) {
+      double s = 0.0;
+      for (int j = 0; j <= i; ++j) s += coef[j] * k[j][e];
+      yi[e] = y[e] + dt * s;
+    }
+    if (post) post(post_user, yi.data());
+    if (stages) std::memcpy(stages + (size_t)i * n, yi.data(), sizeof(double) * n);
+  }
+  std::memcpy(y, yi.data(), sizeof(double) * n);
+  return 0;
+}
+
 int check_params(const ref_params* p) {
   if (!p) return -1;
   if (p->nx < 1 || p->ny < 1 || p->order < 1 || p->order > MAXM) return -1;
   if (!(p->x1 > p->x0) || !(p->y1 > p->y0)) return -1;
-  if (p->rk != 2 && p->rk != 3) return -1;
+  if (p->rk < 2 || p->rk > 5) return -1;
   if (p->bc < 0 || p->bc > 2 || p->eos < 0 || p->eos > 1) return -1;
   if (p->eos == 0 && !(p->gamma > 1.0)) return -1;
   if (p->eos == 1 && !(p->h_aspect > 0.0 && p->gm_star > 0.0)) return -1;
   if (p->damp_r0 > 0.0 && !(p->damp_r1 > p->damp_r0 && p->gm_star > 0.0)) return -1;
+  if (p->limiter != 0 && p->limiter != 1) return -1;
+  if (p->limiter == 1 && !(p->lim_eps > 0.0)) return -1;
   return 0;
 }
 
@@ -367,6 +567,7 @@ int ref_init(const ref_params* p, ref_ctx** out) {
   c->p = *p;
   c->m = p->order;
   build_tables(c->m, &c->T);
+  build_lobatto(c->m, &c->LT);
   c->ncoef = (long)p->ny * p->nx * NV * c->m * c->m;
   c->dx = (p->x1 - p->x0) / p->nx;
   c->dy = (p->y1 - p->y0) / p->ny;
@@ -420,40 +621,110 @@ int ref_cfl_dt(ref_ctx* c, double cfl, double* dt) {
       const double s = (std::fabs(vx) + cs) / c->dx + (std::fabs(vy) + cs) / c->dy;
       if (s > worst) worst = s;
     }
-  *dt = cfl / (2.0 * (m - 1) + 1.0) / worst;
+  double factor = 1.0 / (2.0 * (m - 1) + 1.0);
+  if (p.limiter) factor = std::fmin(factor, 0.5 * c->LT.wh[0]);     /* min(1/(2N_p+1), w_1/2) */
+  *dt = cfl * factor / worst;
   return 0;
 }
 
-/* C8: Shu-Osher form of SSP(2,2) and SSP(3,3) (Gottlieb & Shu 1998).
- * Stage times c = (0,1) and (0,1,1/2). */
-int ref_rk_step(int rk, long n, double* y, double t, double dt, ref_ode_fn f, void* user,
-                double* stages) {
+int ref_rk_stages(int rk) { return rk == 2 ? 2 : rk == 3 ? 3 : rk == 4 ? 5 : rk == 5 ? 6 : -1; }
+
+/* C8: Shu-Osher form of SSP(2,2) and SSP(3,3) (Gottlieb & Shu 1998), stage times
+ * c = (0,1) and (0,1,1/2); rk 4, 5: Butcher form (C8b).  post: applied to every sub-step's result. */
+static int rk_step_impl(int rk, long n, double* y, double t, double dt, ref_ode_fn f, void* user,
+                        double* stages, post_fn post, void* pu) {
+  if (rk == 4 || rk == 5) return butcher_step(rk, n, y, t, dt, f, user, stages, post, pu);
   if (rk != 2 && rk != 3) return -1;
   std::vector<double> L(n), u1(n), u2(n);
   f(user, t, y, L.data());
   for (long k = 0; k < n; ++k) u1[k] = y[k] + dt * L[k];
+  if (post) post(pu, u1.data());
   if (stages) std::memcpy(stages, u1.data(), sizeof(double) * n);
   f(user, t + dt, u1.data(), L.data());
   if (rk == 2) {
     for (long k = 0; k < n; ++k) y[k] = 0.5 * y[k] + 0.5 * (u1[k] + dt * L[k]);
+    if (post) post(pu, y);
     if (stages) std::memcpy(stages + n, y, sizeof(double) * n);
     return 0;
   }
   for (long k = 0; k < n; ++k) u2[k] = 0.75 * y[k] + 0.25 * (u1[k] + dt * L[k]);
+  if (post) post(pu, u2.data());
   if (stages) std::memcpy(stages + n, u2.data(), sizeof(double) * n);
   f(user, t + 0.5 * dt, u2.data(), L.data());
   for (long k = 0; k < n; ++k) y[k] = (1.0 / 3.0) * y[k] + (2.0 / 3.0) * (u2[k] + dt * L[k]);
+  if (post) post(pu, y);
   if (stages) std::memcpy(stages + 2 * n, y, sizeof(double) * n);
   return 0;
 }
 
+int ref_rk_step(int rk, long n, double* y, double t, double dt, ref_ode_fn f, void* user,
+                double* stages) {
+  return rk_step_impl(rk, n, y, t, dt, f, user, stages, nullptr, nullptr);
+}
+
+static void limiter_hook(void* user, double* y) {
+  const ref_ctx* c = static_cast<const ref_ctx*>(user);
+  limit_all(c, c->LT, y);
+}
+
+/* one time step: the RK sub-steps (C8 / C8b), each followed by the limiter when it is on
+ * (step (iii)(d)), then the wave damping (C11) */
 int ref_step_debug(ref_ctx* c, double dt, double* stages) {
   if (!c || !c->has_state) return -1;
   RhsClosure cl{c};
-  int e = ref_rk_step(c->p.rk, c->ncoef, c->U.data(), c->t, dt, dg_ode, &cl, stages);
+  int e = rk_step_impl(c->p.rk, c->ncoef, c->U.data(), c->t, dt, dg_ode, &cl, stages,
+                       c->p.limiter ? limiter_hook : nullptr, c);
   if (e) return e;
   damp(c, dt);
   c->t += dt;
+  return 0;
+}
+
+int ref_limit(ref_ctx* c) {
+  if (!c || !c->has_state) return -1;
+  limit_all(c, c->LT, c->U.data());
+  return 0;
+}
+
+int ref_lobatto(int m, double* xh, double* wh) {
+  if (m < 1 || m > MAXM || !xh || !wh) return -1;
+  LimTables LT;
+  build_lobatto(m, &LT);
+  for (int k = 0; k < LT.nh; ++k) { xh[k] = LT.xh[k]; wh[k] = LT.wh[k]; }
+  return LT.nh;
+}
+
+int ref_limit_cell(const ref_params* p, double* u, double* theta) {
+  if (check_params(p) != 0 || !u) return -1;
+  Tables T;
+  LimTables LT;
+  build_tables(p->order, &T);
+  build_lobatto(p->order, &LT);
+  limit_cell(*p, T, LT, u, theta);
+  return 0;
+}
+
+/* C13: specific torque on the planet, Eq.(6) PAPER.md:321-328:
+ *   Gamma = r_p x sum_n G M_n (r_n - r_p) / (|r_n - r_p|^2 + eps_p^2)^(3/2)   (z component),
+ * M_n = (cell average of the density) x (cell area), r_n = the cell centre, planet position at time t. */
+int ref_torque(ref_ctx* c, double t, double* gamma_z) {
+  if (!c || !gamma_z || !c->has_state) return -1;
+  const ref_params& p = c->p;
+  const int m = c->m;
+  const double ang = p.omega_planet * t + p.phase0;
+  const double xp = p.r_planet * std::cos(ang), yp = p.r_planet * std::sin(ang);
+  double ax = 0.0, ay = 0.0;
+  for (int j = 0; j < p.ny; ++j)
+    for (int i = 0; i < p.nx; ++i) {
+      const double Mn = c->U[cell_off(c, i, j)] * c->dx * c->dy;
+      const double ddx = p.x0 + (i + 0.5) * c->dx - xp, ddy = p.y0 + (j + 0.5) * c->dy - yp;
+      const double r2 = ddx * ddx + ddy * ddy + p.eps_planet * p.eps_planet;
+      const double r3 = r2 * std::sqrt(r2);
+      ax += p.gm_star * Mn * ddx / r3;
+      ay += p.gm_star * Mn * ddy / r3;
+    }
+  (void)m;
+  *gamma_z = xp * ay - yp * ax;
   return 0;
 }
 

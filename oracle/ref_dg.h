@@ -25,7 +25,8 @@ typedef struct {
   int32_t nx, ny;            /* uniform Cartesian grid of rectangles K_ij */
   double  x0, x1, y0, y1;
   int32_t order;             /* m = N_p + 1 = 1..5 */
-  int32_t rk;                /* 2: SSP(2,2), 3: SSP(3,3) */
+  int32_t rk;                /* 2: SSP(2,2), 3: SSP(3,3); 4: SSP-RK(5,4), Table 1 PAPER.md:463-471;
+                                5: Cash-Karp, Table 2 PAPER.md:473-482 (Butcher form, Appendix A) */
   int32_t bc;                /* 0 periodic, 1 transmissive, 2 frozen to the initial state */
   int32_t eos;               /* 0 ideal gas p=(gamma-1)e; 1 locally isothermal */
   double  gamma;
@@ -34,6 +35,9 @@ typedef struct {
   double  q_planet, r_planet, eps_planet, omega_planet, phase0; /* planet on a fixed circular orbit */
   double  damp_r0, damp_r1;  /* wave-killing zone r0 < r; r0 <= 0: off */
   double  t0;
+  int32_t limiter;           /* 1: positivity-preserving limiter (Zhang & Shu 2010) after every
+                                RK sub-step and the w_1/2 factor in the time step */
+  double  lim_eps;           /* the limiter's floor for density and pressure (Zhang & Shu use 1e-13) */
 } ref_params;
 
 /* --- the same surface as include/dg.h, prefixed ref_, host memory --- */
@@ -43,7 +47,10 @@ int    ref_get_state(ref_ctx*, double* U);
 int    ref_rhs(ref_ctx*, double t, double* L);     /* L(u) of Eq.(3) divided by the mass, at time t */
 int    ref_cfl_dt(ref_ctx*, double cfl, double* dt);
 int    ref_step(ref_ctx*, double dt);              /* RK step (C8) + damping (C11); t += dt */
-int    ref_step_debug(ref_ctx*, double dt, double* stages); /* also u^(1..k), before damping */
+int    ref_step_debug(ref_ctx*, double dt, double* stages); /* also u^(1..k), before damping; k = ref_rk_stages */
+int    ref_rk_stages(int rk);                      /* sub-steps of the scheme: 2, 3, 5 (rk 4), 6 (rk 5) */
+int    ref_limit(ref_ctx*);                        /* C12 alone: limit the current state in place */
+int    ref_torque(ref_ctx*, double t, double* gamma_z); /* C13: Eq.(6) */
 double ref_time(const ref_ctx*);
 int    ref_set_time(ref_ctx*, double t);
 void   ref_destroy(ref_ctx*);
@@ -63,6 +70,11 @@ int  ref_gravity(const ref_params*, double t, double x, double y, double* g2);
 int  ref_rhs_parts(ref_ctx*, double t, int parts, double* L);
 /* C11 alone. */
 int  ref_damp(ref_ctx*, double dt);
+/* C12 pieces: Gauss-Lobatto nodes on [-1,1] and weights normalised to sum 1 (Zhang & Shu's hat-w)
+ * for the limiter of order m (nh = ceil((m+2)/2) points); returns nh.  xh, wh sized 4. */
+int  ref_lobatto(int m, double* xh, double* wh);
+/* C12 on one cell: u[4][m][m] modal, in place; theta (nullable) receives theta1, theta2. */
+int  ref_limit_cell(const ref_params*, double* u, double* theta);
 /* C8 alone: one RK step of y' = f(t,y) for n unknowns; stages (nullable) receives y^(1..k). */
 typedef void (*ref_ode_fn)(void* user, double t, const double* y, double* dydt);
 int  ref_rk_step(int rk, long n, double* y, double t, double dt, ref_ode_fn f, void* user,

@@ -1,0 +1,312 @@
+"""Pins for the oracle's NEXT rows: C8b Butcher-form RK with the paper's printed
+tableaus, C12 the positivity-preserving limiter (
+Zhang & Shu 2010) and C13 the torque on the planet (Eq.(6)).  None of these
+tests re-types the oracle's formulas: they use the paper's printed digits, closed forms, NumPy's
+Legendre routines, invariants, and hand-worked cells."""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+from numpy.polynomial import legendre as npleg
+
+import oracle
+from paper_1805_01443_b200 import workloads as W
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _tableau(name):
+    d = {}
+    for line in open(os.path.join(GOLD, "rk_tableaus.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        nm, kind, *v = line.split()
+        if nm == name:
+            d[kind] = np.array([float(Fraction(x)) for x in v])
+    s = len(d["c"])
+    A = np.zeros((s, s))
+    for i in range(1, s):
+        A[i, :i] = d[f"a{i}"]
+    return d["c"], A, d["b"]
+
+
+# ------------------------------------------------------------------------------------------------
+# C8b
+@pytest.mark.parametrize("rk,name,s", [(4, "ssp54", 5), (5, "ck65", 6)])
+def test_butcher_coefficients_are_the_papers(rk, name, s):
+    """Recover c, a_ij, b from the integrator itself with y' = l_j(t) (the Lagrange polynomial of
+    stage time j): sub-step i then returns y + dt a_{i+1,j}, the step y + dt b_j."""
+    c, A, b = _tableau(name)
+    assert oracle.rk_stages(rk) == s
+    np.testing.assert_allclose(A.sum(axis=1), c, atol=2e-14)          # row sums = c as printed
+    t0, dt = 0.4, 0.37
+    nodes = t0 + c * dt
+    for j in range(s):
+        def f(t, y, j=j):
+            v = 1.0
+            for k in range(s):
+                if k != j:
+                    v *= (t - nodes[k]) / (nodes[j] - nodes[k])
+            return np.array([v])
+        y, st = oracle.rk_step(rk, np.array([0.0]), t0, dt, f, want_stages=True)
+        for i in range(1, s):
+            assert abs(st[i - 1][0] / dt - A[i, j]) < 1e-13, (i, j)
+        assert abs(y[0] / dt - b[j] / b.sum()) < 1e-13                 # reading G20: b / sum(b)
+        assert abs(y[0] / dt - b[j]) < 1e-10
+    # exact consistency after the renormalisation: y' = 1
+    y = oracle.rk_step(rk, np.array([0.0]), 0.0, 1.0, lambda t, y: np.array([1.0]))
+    assert abs(y[0] - 1.0) < 2e-16
+
+
+@pytest.mark.parametrize("rk,order", [(4, 4), (5, 5)])
+def test_butcher_observed_order(rk, order):
+    """Non-autonomous, nonlinear scalar ODE with a known solution: y = exp(sin t), y' = y cos t."""
+    f = lambda t, y: y * math.cos(t)
+    errs = []
+    for n in (4, 8, 16):
+        y = np.array([1.0])
+        dt = 2.0 / n
+        for k in range(n):
+            y = oracle.rk_step(rk, y, k * dt, dt, f)
+        errs.append(abs(y[0] - math.exp(math.sin(2.0))))
+    rate = math.log2(errs[1] / errs[2])
+    assert abs(rate - order) < 0.35, (errs, rate)
+    # linear ODE: the amplification factor matches exp(z) through z^order
+    z = 0.2
+    y = oracle.rk_step(rk, np.array([1.0]), 0.0, 1.0, lambda t, y: z * y)
+    assert abs(y[0] - math.exp(z)) < 0.02 * z ** (order + 1)
+
+
+@pytest.mark.parametrize("rk,order", [(3, 3), (4, 4), (5, 5)])
+def test_dg_step_temporal_order_by_step_halving(rk, order):
+    """The full DG step on a fixed grid (entropy wave, order 3): successive halvings of dt change the
+    state at T by amounts whose ratio is 2^order -- the time integrator drives the DG operator
+    (stage times, stage states) at its design order."""
+    sols = []
+    for n in (6, 12, 24):
+        p, U = W.entropy_wave(6, 3, rk=rk)
+        r = oracle.RefDG(p)
+        r.set_state(U)
+        for _ in range(n):
+            r.step(0.4 / n)
+        sols.append(r.get_state())
+    d1 = np.abs(sols[0] - sols[1]).max()
+    d2 = np.abs(sols[1] - sols[2]).max()
+    assert abs(math.log2(d1 / d2) - order) < 0.5, (d1, d2)
+
+
+# ------------------------------------------------------------------------------------------------
+# C12
+def test_lobatto_closed_forms_and_exactness():
+    assert [len(oracle.lobatto(m)[0]) for m in (1, 2, 3, 4, 5)] == [2, 2, 3, 3, 4]
+    x, w = oracle.lobatto(2)
+    np.testing.assert_allclose(x, [-1, 1], atol=0)
+    np.testing.assert_allclose(w, [0.5, 0.5], atol=1e-16)
+    x, w = oracle.lobatto(3)
+    np.testing.assert_allclose(x, [-1, 0, 1], atol=0)
+    np.testing.assert_allclose(w, [1 / 6, 2 / 3, 1 / 6], atol=1e-16)
+    x, w = oracle.lobatto(5)
+    np.testing.assert_allclose(x, [-1, -1 / math.sqrt(5), 1 / math.sqrt(5), 1], atol=1e-16)
+    np.testing.assert_allclose(w, [1 / 12, 5 / 12, 5 / 12, 1 / 12], atol=1e-16)
+    for m in (1, 2, 3, 4, 5):
+        x, w = oracle.lobatto(m)
+        assert 2 * len(x) - 3 >= m - 1                   # exact for the cell polynomials' degree N_p
+        for k in range(2 * len(x) - 2):
+            exact = 0.0 if k % 2 else 1.0 / (k + 1)      # (1/2) int_-1^1 x^k
+            assert abs((w * x ** k).sum() - exact) < 1e-15
+
+
+def _cell_values(u, px, py):
+    """u[v][b][a] evaluated at the tensor points (px_i, py_j) with NumPy's Legendre routines."""
+    m = u.shape[-1]
+    nrm = np.sqrt(2 * np.arange(m) + 1.0)
+    c = u * nrm[None, :, None] * nrm[None, None, :]       # coefficients of P_b(y) P_a(x)
+    # legval2d(x, y, c): c[i, j] multiplies L_i(x) L_j(y); our c is [b][a] -> transpose
+    return np.stack([npleg.leggrid2d(px, py, c[v].T) for v in range(u.shape[0])])   # [v][ix][iy]
+
+
+def _limiter_point_values(m, u):
+    xg = npleg.leggauss(m)[0]
+    xh, _ = oracle.lobatto(m)
+    a = _cell_values(u, xg, xh).reshape(4, -1)            # Gauss in x, Lobatto in y
+    b = _cell_values(u, xh, xg).reshape(4, -1)            # Lobatto in x, Gauss in y
+    return np.concatenate([a, b], axis=1)
+
+
+@pytest.mark.parametrize("m", [2, 3, 4, 5])
+def test_cell_average_is_a_convex_combination_of_the_limiter_points(m):
+    """Zhang & Shu's decomposition: ubar = sum_q sum_k (w_q/2) what_k u(x_q, xh_k), both ways round,
+    with positive weights -- the reason these are the points where positivity is enforced."""
+    rng = np.random.default_rng(m)
+    u = rng.standard_normal((4, m, m))
+    xg, wg = npleg.leggauss(m)
+    xh, wh = oracle.lobatto(m)
+    assert (wh > 0).all()
+    a = _cell_values(u, xg, xh)
+    b = _cell_values(u, xh, xg)
+    np.testing.assert_allclose(np.einsum("vqk,q,k->v", a, wg / 2, wh), u[:, 0, 0], atol=1e-14)
+    np.testing.assert_allclose(np.einsum("vkq,q,k->v", b, wg / 2, wh), u[:, 0, 0], atol=1e-14)
+
+
+def _pressure(s, gamma=1.4):
+    return (gamma - 1) * (s[3] - 0.5 * (s[1] ** 2 + s[2] ** 2) / s[0])
+
+
+@pytest.mark.parametrize("m", [2, 3, 4, 5])
+def test_limiter_invariants_on_random_cells(m):
+    rng = np.random.default_rng(100 + m)
+    p = W.make_params(nx=1, ny=1, order=m, eos=0, gamma=1.4, limiter=1, lim_eps=1e-8)
+    n_dens = n_pres = 0
+    for trial in range(60):
+        u = 0.6 * rng.standard_normal((4, m, m)) / (1 + np.arange(m)[:, None] + np.arange(m)[None, :])
+        u[:, 0, 0] = [1.0, 0.3, -0.2, 1.5]               # admissible average: p = 0.4 (1.5 - 0.065)
+        if trial % 3 == 0:
+            u[:, 1:, :] *= 0.05
+            u[:, :, 1:] *= 0.05                          # nearly constant: admissible, must be untouched
+        before = _limiter_point_values(m, u)
+        lim, th1, th2 = oracle.limit_cell(p, u)
+        np.testing.assert_array_equal(lim[:, 0, 0], u[:, 0, 0])      # averages kept bitwise
+        after = _limiter_point_values(m, lim)
+        assert after[0].min() >= 1e-8 * (1 - 1e-9)
+        assert _pressure(after).min() >= 1e-8 * (1 - 1e-6) - 1e-15
+        admissible = before[0].min() >= 1e-8 and _pressure(before).min() >= 1e-8
+        if admissible:
+            np.testing.assert_array_equal(lim, u)
+            assert th1 == 1.0 and th2 == 1.0
+        if th1 < 1.0:
+            n_dens += 1
+            if th2 == 1.0:
+                assert abs(after[0].min() - 1e-8) < 1e-13         # the worst point lands on eps
+                np.testing.assert_allclose(lim[0].ravel()[1:], th1 * u[0].ravel()[1:], rtol=1e-15)
+        if th2 < 1.0:
+            n_pres += 1
+            assert abs(_pressure(after).min() - 1e-8) < 1e-11         # the binding point has p = eps
+    assert n_dens > 5 and n_pres > 5
+
+
+def test_limiter_hand_worked_cells():
+    """m = 2: phi_1(-1) = -sqrt(3).  (i) rho = 1 + a phi_1(xi): theta1 = (1 - eps)/(a sqrt 3).
+    (ii) rho = 1, m = 0, E = 1 + e phi_1(xi): p linear along the segment, theta2 = (1 - eps/0.4)/(e sqrt 3).
+    (iii) rho = 1, E = 1, m_x = c phi_1(xi): p = 0.4 (1 - 3 c^2 t^2 / 2) -> theta2 = sqrt((1 - eps/0.4) 2/(3 c^2))."""
+    eps = 1e-6
+    p = W.make_params(nx=1, ny=1, order=2, eos=0, gamma=1.4, limiter=1, lim_eps=eps)
+    s3 = math.sqrt(3.0)
+    u = np.zeros((4, 2, 2)); u[:, 0, 0] = [1, 0, 0, 1]; u[0, 0, 1] = 0.9
+    lim, th1, th2 = oracle.limit_cell(p, u)
+    assert abs(th1 - (1 - eps) / (0.9 * s3)) < 1e-15 and th2 == 1.0
+    u = np.zeros((4, 2, 2)); u[:, 0, 0] = [1, 0, 0, 1]; u[3, 0, 1] = 0.8
+    lim, th1, th2 = oracle.limit_cell(p, u)
+    assert th1 == 1.0 and abs(th2 - (1 - eps / 0.4) / (0.8 * s3)) < 1e-14
+    u = np.zeros((4, 2, 2)); u[:, 0, 0] = [1, 0, 0, 1]; u[1, 0, 1] = 1.1
+    lim, th1, th2 = oracle.limit_cell(p, u)
+    assert th1 == 1.0 and abs(th2 - math.sqrt((1 - eps / 0.4) * 2 / (3 * 1.1 ** 2))) < 1e-14
+    # y-direction twin of (i): the Lobatto points in y are in the set as well
+    u = np.zeros((4, 2, 2)); u[:, 0, 0] = [1, 0, 0, 1]; u[0, 1, 0] = -0.9
+    lim, th1, th2 = oracle.limit_cell(p, u)
+    assert abs(th1 - (1 - eps) / (0.9 * s3)) < 1e-15
+
+
+def test_limiter_isothermal_only_touches_density():
+    p = W.make_params(nx=1, ny=1, order=3, eos=1, h_aspect=0.05, gm_star=1.0, eps_star=0.1, limiter=1, lim_eps=1e-10)
+    rng = np.random.default_rng(5)
+    u = rng.standard_normal((4, 3, 3))
+    u[0, 0, 0] = 0.3
+    lim, th1, th2 = oracle.limit_cell(p, u)
+    assert th1 < 1.0 and th2 == 1.0
+    np.testing.assert_array_equal(lim[1:], u[1:])
+    assert _limiter_point_values(3, lim)[0].min() >= 1e-10 * (1 - 1e-6)
+
+
+def test_limiter_time_step_factor():
+    """dt = C min(1/(2N_p+1), w_1/2) (...)^-1 with w_1 the first Gauss-Lobatto weight."""
+    for m, w1 in ((2, 0.5), (3, 1 / 6), (4, 1 / 6), (5, 1 / 12)):
+        p, U = W.vortex(4, m)
+        r0 = oracle.RefDG(p); r0.set_state(U)
+        r1 = oracle.RefDG(dict(p, limiter=1)); r1.set_state(U)
+        ratio = r1.cfl_dt(0.2) / r0.cfl_dt(0.2)
+        assert abs(ratio - min(1 / (2 * m - 1), w1 / 2) * (2 * m - 1)) < 1e-15
+
+
+def test_limiter_is_applied_after_every_substep_and_keeps_mass():
+    """A state with an under-resolved density dip: with the limiter every sub-step result is admissible
+    at the limiter's points, mass is conserved to round-off (periodic, no gravity), and on smooth
+    data the limited and unlimited steps are bitwise identical."""
+    p, U = W.random_smooth(6, 5, 3, seed=3, bc=0, rk=3)
+    U[2, 3, 0, 0, 1] = 0.9                                # rho dips below zero at the cell's west edge
+    pl = dict(p, limiter=1, lim_eps=1e-10)
+    r = oracle.RefDG(pl)
+    r.set_state(U)
+    r.limit()
+    dt = 0.5 * r.cfl_dt(0.2)
+    st = r.step_debug(dt)
+    for s in range(3):
+        for j in range(5):
+            for i in range(6):
+                v = _limiter_point_values(3, st[s, j, i])
+                assert v[0].min() >= 1e-10 * (1 - 1e-6) and _pressure(v).min() >= 1e-10 * (1 - 1e-4)
+    np.testing.assert_allclose(st[-1][..., 0, 0].sum(axis=(0, 1)), U[..., 0, 0].sum(axis=(0, 1)), rtol=1e-14)
+    p2, U2 = W.random_smooth(6, 5, 3, seed=3, bc=0, rk=3)
+    a = oracle.RefDG(p2); a.set_state(U2); a.step(dt)
+    b = oracle.RefDG(dict(p2, limiter=1)); b.set_state(U2); b.step(dt)
+    np.testing.assert_array_equal(a.get_state(), b.get_state())
+
+
+# ------------------------------------------------------------------------------------------------
+# C13
+def _torque_setup(n=12, m=2):
+    p = W.make_params(nx=n, ny=n, order=m, x0=-2.0, x1=2.0, y0=-2.0, y1=2.0, eos=0, gamma=1.4,
+                      gm_star=1.0, eps_star=0.0, q_planet=1e-3, r_planet=1.0, eps_planet=0.1,
+                      omega_planet=1.0, phase0=0.3)
+    return p
+
+
+def test_torque_is_minus_dPhi_dphi_of_the_cells_potential():
+    """Gamma_z = (r_p x g)_z = -d Phi/d phi with Phi(phi) = -sum_n G M_n / sqrt(|r_n - r_p(phi)|^2 + eps^2):
+    centred finite difference of the potential along the orbit, against Eq.(6)."""
+    p = _torque_setup()
+    rng = np.random.default_rng(0)
+    n, m = p["nx"], p["order"]
+    U = rng.standard_normal((n, n, 4, m, m))               # higher modes must not matter
+    U[..., 0, 0, 0] = rng.uniform(0.5, 2.0, size=(n, n))
+    r = oracle.RefDG(p)
+    r.set_state(U)
+    dx = 4.0 / n
+    xc = -2.0 + (np.arange(n) + 0.5) * dx
+    M = U[..., 0, 0, 0] * dx * dx
+
+    def Phi(ang):
+        xp, yp = math.cos(ang), math.sin(ang)
+        d2 = (xc[None, :] - xp) ** 2 + (xc[:, None] - yp) ** 2 + 0.1 ** 2
+        return -(M / np.sqrt(d2)).sum()
+
+    t = 0.8
+    ang = 1.0 * t + 0.3
+    h = 1e-5
+    fd = -(Phi(ang + h) - Phi(ang - h)) / (2 * h)
+    assert abs(r.torque(t) - fd) < 1e-8 * max(1.0, abs(fd))
+
+
+def test_torque_symmetries():
+    p = dict(_torque_setup(), phase0=0.0)
+    n, m = p["nx"], p["order"]
+    rng = np.random.default_rng(1)
+    U = np.zeros((n, n, 4, m, m))
+    rho = rng.uniform(0.5, 2.0, size=(n, n))
+    U[..., 0, 0, 0] = rho + rho[::-1, :]                   # symmetric about the x axis, planet on it
+    r = oracle.RefDG(p); r.set_state(U)
+    assert abs(r.torque(0.0)) < 1e-14
+    U[..., 0, 0, 0] = rho
+    r.set_state(U); g1 = r.torque(0.0)
+    U[..., 0, 0, 0] = rho[::-1, :]
+    r.set_state(U); g2 = r.torque(0.0)
+    assert abs(g1 + g2) < 1e-14 * max(1, abs(g1)) and abs(g1) > 1e-3
+    # one massive cell, by hand: M at (xc, yc), planet at (1, 0): Gamma = x_p a_y = M yc / d^3
+    U[:] = 0.0
+    U[9, 7, 0, 0, 0] = 3.0
+    r.set_state(U)
+    dx = 4.0 / n
+    xcell, ycell = -2 + 7.5 * dx, -2 + 9.5 * dx
+    d3 = ((xcell - 1) ** 2 + ycell ** 2 + 0.01) ** 1.5
+    assert abs(r.torque(0.0) - 3.0 * dx * dx * ycell / d3) < 1e-15
