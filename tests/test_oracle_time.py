@@ -19,7 +19,8 @@ def _tableaus():
         if line.startswith("#") or not line.strip():
             continue
         name, kind, *v = line.split()
-        d[(name, kind)] = np.array([float(x) for x in v])
+        if name in ("ssp22", "ssp33"):
+            d[(name, kind)] = np.array([float(x) for x in v])
     return d
 
 
