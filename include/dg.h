@@ -43,7 +43,10 @@ typedef struct {
   int32_t nx, ny;                 /* cells K_ij = [x_{i-1/2},x_{i+1/2}] x [y_{j-1/2},y_{j+1/2}] */
   double  x0, x1, y0, y1;         /* domain; dx = (x1-x0)/nx, dy = (y1-y0)/ny */
   int32_t order;                  /* m = 1..5: m x m modes per cell and variable */
-  int32_t rk;                     /* 2: SSP-RK(2,2), 3: SSP-RK(3,3) (Gottlieb & Shu 1998) */
+  int32_t rk;                     /* 2: SSP-RK(2,2), 3: SSP-RK(3,3) (Gottlieb & Shu 1998);
+                                     4: the five-stage fourth-order SSP scheme of Table 1,
+                                     5: the six-stage Cash-Karp scheme of Table 2, both in
+                                     Butcher form (Appendix A); see dg_rk_stages */
   int32_t bc;                     /* 0 periodic; 1 transmissive (exterior trace = interior);
                                      2 frozen: exterior trace = trace of the state given to the last
                                      dg_set_state*, same boundary cell, same face point */
@@ -58,6 +61,10 @@ typedef struct {
                                      no indirect term; q = 0: no planet */
   double  damp_r0, damp_r1;       /* wave-killing zone r0 < r (<= r1 and beyond); r0 <= 0: off */
   double  t0;                     /* initial time */
+  int32_t limiter;                /* 1: positivity-preserving limiter (Zhang & Shu 2010) after
+                                     every RK sub-step (step (iii)(d)), and dg_cfl_dt uses the factor
+                                     min(1/(2N_p+1), w_1/2) of PAPER.md:131; 0: off */
+  double  lim_eps;                /* limiter floor for density and pressure (> 0 when limiter = 1; 1e-13) */
 } dg_params;
 
 /* Bytes of DEVICE workspace dg_init needs for these parameters (0 if they are invalid). */
@@ -95,9 +102,28 @@ int dg_cfl_dt(dg_ctx*, double cfl, double* dt /*HOST*/);
  * relaxation Q <- (dt Q0 + tau Q)/(tau + dt) if enabled; t += dt. */
 int dg_step(dg_ctx*, double dt);
 
-/* Same, and also writes the rk stage states u^(1..k) (before damping), modal layout,
- * stages: [rk][ny][nx][4][m][m] DEVICE.  For per-stage parity tests. */
+/* Same, and also writes the results of the k = dg_rk_stages(rk) sub-steps (after the limiter, before
+ * damping; the last one is u^{n+1}), modal layout, stages: [k][ny][nx][4][m][m] DEVICE.  For per-stage
+ * parity tests. */
 int dg_step_debug(dg_ctx*, double dt, double* stages /*DEVICE*/);
+
+/* Sub-steps (right-hand-side evaluations) per time step of scheme rk: 2, 3, 5 (rk 4), 6 (rk 5); -1 if unknown. */
+int dg_rk_stages(int rk);
+
+/* Apply the positivity-preserving limiter (Zhang & Shu 2010) to the current state, in
+ * place, with floor lim_eps -- whether or not params.limiter is set (e.g. on a freshly projected initial
+ * state).  Cell averages are unchanged.  Per cell K, with S_K = (Gauss_m x Lobatto_nh) U (Lobatto_nh x Gauss_m),
+ * nh the smallest Gauss-Lobatto rule exact for degree N_p:
+ *   theta1 = min(1, (rho_bar - eps)/(rho_bar - min_S rho)) scales the density's non-constant part; then
+ *   (eos 0) theta2 = min over the points of S_K with p < eps of the parameter t at which the segment
+ *   u_bar + t (u(x) - u_bar) meets p = eps, and scales all four variables' non-constant parts. */
+int dg_limit(dg_ctx*);
+
+/* Specific torque on the planet at time t, Eq.(6) PAPER.md:321-328 (z component):
+ *   Gamma = r_p x sum_n G M_n (r_n - r_p) / (|r_n - r_p|^2 + eps_p^2)^(3/2),
+ * M_n = cell-average density x cell area, r_n = cell centre, G = gm_star (unit stellar mass).
+ * Synchronises the stream and writes one HOST double. */
+int dg_torque(dg_ctx*, double t, double* gamma_z /*HOST*/);
 
 /* Convenience for end-to-end runs from HOST buffers: set_state_host(U_in), then nsteps times
  * { dg_cfl_dt(cfl); dg_step(dt) }, then get_state_host(U_out).  Blocking. */

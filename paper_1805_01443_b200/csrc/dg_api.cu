@@ -14,6 +14,7 @@
 #include "dg_tables.h"
 #include "dg_kernels.cuh"
 #include "dg_stage_launch.cuh"
+#include "dg_limit.cuh"
 
 using namespace dg;
 
@@ -26,14 +27,17 @@ struct Layout {
   size_t state_doubles;      // ny * nbx * 4 m^2 * 32
   size_t state_bytes;
   bool need_q0, need_btr;
-  size_t off_q[3], off_q0, off_btrW, off_btrE, off_btrS, off_btrN, off_scalars, total;
+  int nkbuf;                 // slope buffers K_j of the Butcher-form schemes (rk 4: 4, rk 5: 5)
+  size_t off_q[3], off_k[MAXK], off_q0, off_btrW, off_btrE, off_btrS, off_btrN, off_partial, off_scalars, total;
 };
 
 bool valid_params(const dg_params* p) {
   if (!p) return false;
   if (p->nx < 1 || p->ny < 1 || p->order < 1 || p->order > MAXM) return false;
   if (!(p->x1 > p->x0) || !(p->y1 > p->y0)) return false;
-  if (p->rk != 2 && p->rk != 3) return false;
+  if (p->rk < 2 || p->rk > 5) return false;
+  if (p->limiter != 0 && p->limiter != 1) return false;
+  if (p->limiter == 1 && !(p->lim_eps > 0.0)) return false;
   if (p->bc < 0 || p->bc > 2 || p->eos < 0 || p->eos > 1) return false;
   if (p->eos == 0 && !(p->gamma > 1.0)) return false;
   if (p->eos == 1 && !(p->h_aspect > 0.0 && p->gm_star > 0.0)) return false;
@@ -52,6 +56,8 @@ Layout make_layout(const dg_params* p) {
   L.need_btr = p->bc == 2;
   size_t off = 0;
   for (int k = 0; k < 3; ++k) { L.off_q[k] = off; off += L.state_bytes; }
+  L.nkbuf = p->rk == 4 ? 4 : (p->rk == 5 ? 5 : 0);
+  for (int k = 0; k < MAXK; ++k) { L.off_k[k] = off; if (k < L.nkbuf) off += L.state_bytes; }
   L.off_q0 = off;
   if (L.need_q0) off += L.state_bytes;
   const size_t side = align_up((size_t)p->ny * 4 * L.m * sizeof(double));
@@ -60,6 +66,8 @@ Layout make_layout(const dg_params* p) {
   L.off_btrE = off; if (L.need_btr) off += side;
   L.off_btrS = off; if (L.need_btr) off += top;
   L.off_btrN = off; if (L.need_btr) off += top;
+  // torque partial sums: 2 doubles per block of torque_kernel
+  L.off_partial = off; off += align_up((size_t)L.nbx * ((p->ny + 3) / 4) * 2 * sizeof(double));
   L.off_scalars = off; off += ALIGN;
   L.total = off;
   return L;
@@ -70,6 +78,8 @@ struct dg_ctx {
   dg_params p;
   Layout L;
   HostTables H;
+  HostLimTables HL;
+  LimDev LD;
   DevTables T;
   ConvTables CT;
   Geom g;
@@ -88,6 +98,8 @@ struct dg_ctx {
   std::string err;
 
   double* q(int k) const { return reinterpret_cast<double*>(ws + L.off_q[k]); }
+  double* kbuf(int k) const { return reinterpret_cast<double*>(ws + L.off_k[k]); }
+  double* partial() const { return reinterpret_cast<double*>(ws + L.off_partial); }
   double* q0() const { return reinterpret_cast<double*>(ws + L.off_q0); }
   double* btrW() const { return reinterpret_cast<double*>(ws + L.off_btrW); }
   double* btrE() const { return reinterpret_cast<double*>(ws + L.off_btrE); }
@@ -145,10 +157,23 @@ Phys make_phys(const dg_ctx* c, double t, double beta = 1.0) {
 // dg_kernels.cuh; K_RHS writes L itself).  The kernel computes a*qn + b*qprev + beta*L with
 // beta = b*dt folded into the derivative / lifting tables and the gravity constants here; the
 // lifting vectors also carry the 1/2 of the Lax-Friedrichs average (the kernel forms 2 x flux).
+struct GenArgs {               // K_GEN / K_GENL: out = u^n + sum_j kc[j] kin[j] + kself K_i, K_i = dt N -> kout
+  int nk;
+  const double* kin[MAXK];
+  double kc[MAXK];
+  double kself;
+  double* kout;
+};
+
 int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout, double a, double b,
-                 double dt, double t, int kind) {
+                 double dt, double t, int kind, const GenArgs* ga = nullptr) {
   StageArgs A{};
-  const double beta = kind == K_RHS ? 1.0 : b * dt;
+  const bool gen = kind == K_GEN || kind == K_GENL;
+  const double beta = kind == K_RHS ? 1.0 : (gen ? dt : b * dt);
+  if (gen) {
+    A.nk = ga->nk; A.kself = ga->kself; A.kout = ga->kout;
+    for (int k = 0; k < ga->nk; ++k) { A.kin[k] = ga->kin[k]; A.kc[k] = ga->kc[k]; }
+  }
   A.qprev = qprev; A.qn = qn; A.qout = qout; A.q0 = c->q0();
   A.btrW = c->btrW(); A.btrE = c->btrE(); A.btrS = c->btrS(); A.btrN = c->btrN();
   A.wmax = c->wmax();
@@ -266,6 +291,59 @@ int launch_damp(dg_ctx* c, double* Q, double dt) {
   return DG_OK;
 }
 
+template <typename F>
+void dispatch_m_tag(int m, F f) {
+  switch (m) {
+    case 1: f(std::integral_constant<int, 1>{}); break;
+    case 2: f(std::integral_constant<int, 2>{}); break;
+    case 3: f(std::integral_constant<int, 3>{}); break;
+    case 4: f(std::integral_constant<int, 4>{}); break;
+    default: f(std::integral_constant<int, 5>{});
+  }
+}
+
+// Positivity limiter on Q in place (row NEXT-1).  final_: also the wave-killing relaxation with this
+// step's dt and the CFL reduction of the result (the work the last stage kernel does when the
+// limiter is off; the limiter has to come between them, PAPER.md:150 then PAPER.md:292).
+int launch_limit(dg_ctx* c, double* Q, bool final_, double dt) {
+  LimitArgs A{};
+  A.q = Q; A.q0 = c->q0(); A.wmax = c->wmax();
+  A.eps = c->p.lim_eps > 0.0 ? c->p.lim_eps : 1e-13;
+  A.dt = dt;
+  const bool damp = final_ && c->p.damp_r0 > 0.0;
+  A.damp_r0 = damp ? c->p.damp_r0 : 0.0;
+  A.damp_inv_w = damp ? 1.0 / (c->p.damp_r1 - c->p.damp_r0) : 0.0;
+  A.damp_tau0 = damp ? 2.0 * 3.14159265358979323846 *
+                           std::sqrt(c->p.damp_r0 * c->p.damp_r0 * c->p.damp_r0 / c->p.gm_star)
+                     : 0.0;
+  A.rows = c->rows_per_cta;
+  A.g = c->g;
+  A.ph = make_phys(c, c->t);
+  A.LT = c->LD;
+  dim3 grid(c->L.nbx, (c->p.ny + A.rows - 1) / A.rows);
+  cudaStream_t s = c->stream;
+  const int eos = c->p.eos;
+  cudaError_t err = cudaSuccess;
+  dispatch_m_tag(c->L.m, [&](auto tag) {
+    constexpr int M = decltype(tag)::value;
+    constexpr size_t smem = limit_smem_bytes<M>();
+    auto go = [&](auto kern) {
+      err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (err == cudaSuccess) kern<<<grid, M * 32, smem, s>>>(A);
+    };
+    if (eos == 0) { if (final_) go(limit_kernel<M, 0, true>); else go(limit_kernel<M, 0, false>); }
+    else          { if (final_) go(limit_kernel<M, 1, true>); else go(limit_kernel<M, 1, false>); }
+  });
+  c->launches++;
+  if (err != cudaSuccess) return fail(c, DG_ECUDA, "limit kernel launch", err);
+  CUDA_TRY(c, cudaGetLastError());
+  return DG_OK;
+}
+
+// One time step.  Sub-step results are limited when the limiter is on; the wave-killing
+// relaxation and the CFL reduction for the next step ride on the last kernel of the step: the last
+// stage kernel (limiter off) or the last limiter pass (limiter on).  With `stages` (debug path) they
+// run as their own passes so that the recorded sub-step results are "before damping".
 int do_step(dg_ctx* c, double dt, double* stages) {
   if (!c) return DG_EINVAL;
   if (!c->has_state) return fail(c, DG_ESTATE, "dg_step: state not set");
@@ -273,29 +351,58 @@ int do_step(dg_ctx* c, double dt, double* stages) {
   const int A = c->cur, B = (c->cur + 1) % 3, Cc = (c->cur + 2) % 3;
   const size_t n = (size_t)c->p.ny * c->p.nx * 4 * c->L.m * c->L.m;
   const bool damp = c->p.damp_r0 > 0.0;
-  // the fused reduction rides on the last stage (K_LAST*); with DG_TUNE_FUSED_CFL = 0 or in the debug
-  // path (stages are "before damping": damping runs as its own pass below) the last stage is plain
-  int last = damp ? K_LASTD : K_LAST;
-  if (stages || (!c->fused_cfl && !damp)) last = K_MID;
+  const bool lim = c->p.limiter != 0;
+  const bool fuse_tail = !stages && (c->fused_cfl || damp);   // damping + CFL ride on the step's last kernel
   int e;
-  if (c->fused_cfl && !stages)
-    CUDA_TRY(c, cudaMemsetAsync(c->wmax(), 0, sizeof(unsigned long long), c->stream));
-  // SSP-RK in Shu-Osher form, stage times c = (0,1) / (0,1,1/2)
-  if ((e = launch_stage(c, c->q(A), c->q(A), c->q(B), 0.0, 1.0, dt, c->t, K_FIRST))) return e;
-  if (stages && (e = to_modal(c, c->q(B), stages))) return e;
-  if (c->p.rk == 2) {
-    if ((e = launch_stage(c, c->q(B), c->q(A), c->q(Cc), 0.5, 0.5, dt, c->t + dt, last))) return e;
-    if (stages && (e = to_modal(c, c->q(Cc), stages + n))) return e;
-    c->cur = Cc;
+  if (fuse_tail) CUDA_TRY(c, cudaMemsetAsync(c->wmax(), 0, sizeof(unsigned long long), c->stream));
+  // after every sub-step: limiter, then (debug) the copy-out
+  auto after = [&](double* Q, int k, bool last) -> int {
+    int err = DG_OK;
+    if (lim) err = launch_limit(c, Q, last && fuse_tail, dt);
+    if (!err && stages) err = to_modal(c, Q, stages + (size_t)k * n);
+    return err;
+  };
+  if (c->p.rk <= 3) {
+    // SSP-RK in Shu-Osher form, stage times c = (0,1) / (0,1,1/2)
+    const int last = (fuse_tail && !lim) ? (damp ? K_LASTD : K_LAST) : K_MID;
+    if ((e = launch_stage(c, c->q(A), c->q(A), c->q(B), 0.0, 1.0, dt, c->t, K_FIRST))) return e;
+    if ((e = after(c->q(B), 0, false))) return e;
+    if (c->p.rk == 2) {
+      if ((e = launch_stage(c, c->q(B), c->q(A), c->q(Cc), 0.5, 0.5, dt, c->t + dt, last))) return e;
+      if ((e = after(c->q(Cc), 1, true))) return e;
+      c->cur = Cc;
+    } else {
+      if ((e = launch_stage(c, c->q(B), c->q(A), c->q(Cc), 0.75, 0.25, dt, c->t + dt, K_MID))) return e;
+      if ((e = after(c->q(Cc), 1, false))) return e;
+      if ((e = launch_stage(c, c->q(Cc), c->q(A), c->q(B), 1.0 / 3.0, 2.0 / 3.0, dt, c->t + 0.5 * dt, last))) return e;
+      if ((e = after(c->q(B), 2, true))) return e;
+      c->cur = B;
+    }
   } else {
-    if ((e = launch_stage(c, c->q(B), c->q(A), c->q(Cc), 0.75, 0.25, dt, c->t + dt, K_MID))) return e;
-    if (stages && (e = to_modal(c, c->q(Cc), stages + n))) return e;
-    if ((e = launch_stage(c, c->q(Cc), c->q(A), c->q(B), 1.0 / 3.0, 2.0 / 3.0, dt, c->t + 0.5 * dt, last))) return e;
-    if (stages && (e = to_modal(c, c->q(B), stages + 2 * n))) return e;
-    c->cur = B;
+    // Butcher form (Appendix A): y_{i+1} = u^n + sum_{j<=i} a_{i+1,j} K_j, K_j = dt N(y_j, t_j),
+    // the last row being b.  Sub-step i reads y_i (with halo), u^n and the earlier K_j, writes K_i and y_{i+1}.
+    ButcherTableau bt;
+    butcher_tableau(c->p.rk, &bt);
+    int in = A, out = B;
+    for (int i = 0; i < bt.s; ++i) {
+      const bool last = i + 1 == bt.s;
+      const double* coef = last ? bt.b : bt.a[i + 1];
+      GenArgs ga{};
+      for (int j = 0; j < i; ++j)
+        if (coef[j] != 0.0) { ga.kin[ga.nk] = c->kbuf(j); ga.kc[ga.nk] = coef[j]; ga.nk++; }
+      ga.kself = coef[i];
+      ga.kout = last ? nullptr : c->kbuf(i);
+      const int kind = (last && fuse_tail && !lim) ? K_GENL : K_GEN;
+      // without the fused tail K_GENL must not damp: K_GEN never does
+      if ((e = launch_stage(c, c->q(in), c->q(A), c->q(out), 0.0, 0.0, dt, c->t + bt.c[i] * dt, kind, &ga))) return e;
+      if ((e = after(c->q(out), i, last))) return e;
+      in = out;
+      out = (out == B) ? Cc : B;
+    }
+    c->cur = in;
   }
-  c->wmax_valid = c->fused_cfl && last >= K_LAST;
-  if (stages && damp) {   // debug path: stages are "before damping", so relax in a separate pass
+  c->wmax_valid = fuse_tail && c->fused_cfl;
+  if (!fuse_tail && damp) {   // damping as its own pass (debug path, or nothing to ride on)
     if ((e = launch_damp(c, c->q(c->cur), dt))) return e;
   }
   c->t += dt;
@@ -334,6 +441,12 @@ int dg_init(const dg_params* p, void* workspace, size_t ws_bytes, void* cuda_str
   c->timing = false;
   c->ev_used = 0;
   build_host_tables(p->order, &c->H);
+  build_limiter_tables(p->order, &c->HL);
+  std::memset(&c->LD, 0, sizeof c->LD);
+  c->LD.nh = c->HL.nh;
+  for (int k = 0; k < c->HL.nh; ++k)
+    for (int r = 0; r < p->order; ++r) c->LD.Lh[k][r] = c->HL.Lh[k][r];
+  for (int r = 0; r < p->order; ++r) c->LD.w[r] = c->H.w[r];
   Geom& g = c->g;
   g.x0 = p->x0; g.y0 = p->y0;
   g.dx = (p->x1 - p->x0) / p->nx; g.dy = (p->y1 - p->y0) / p->ny;
@@ -429,7 +542,41 @@ int dg_cfl_dt(dg_ctx* c, double cfl, double* dt) {
   double worst = 0.0;
   CUDA_TRY(c, cudaMemcpyAsync(&worst, c->wmax(), sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-  *dt = cfl / (2.0 * (c->L.m - 1) + 1.0) / worst;
+  double factor = 1.0 / (2.0 * (c->L.m - 1) + 1.0);
+  if (c->p.limiter) factor = std::fmin(factor, 0.5 * c->HL.w1);
+  *dt = cfl * factor / worst;
+  return DG_OK;
+}
+
+int dg_rk_stages(int rk) { return rk == 2 ? 2 : rk == 3 ? 3 : rk == 4 ? 5 : rk == 5 ? 6 : -1; }
+
+int dg_limit(dg_ctx* c) {
+  if (!c) return DG_EINVAL;
+  if (!c->has_state) return fail(c, DG_ESTATE, "dg_limit: state not set");
+  c->wmax_valid = false;
+  return launch_limit(c, c->q(c->cur), false, 0.0);
+}
+
+int dg_torque(dg_ctx* c, double t, double* gamma_z) {
+  if (!c || !gamma_z) return c ? fail(c, DG_EINVAL, "dg_torque: null") : DG_EINVAL;
+  if (!c->has_state) return fail(c, DG_ESTATE, "dg_torque: state not set");
+  const Phys ph = make_phys(c, t);
+  dim3 grid(c->L.nbx, (c->p.ny + 3) / 4);
+  const int nblocks = (int)(grid.x * grid.y);
+  cudaStream_t s = c->stream;
+  const double* Q = c->q(c->cur);
+  double* out = reinterpret_cast<double*>(c->ws + c->L.off_scalars + 128);
+  dispatch_m_tag(c->L.m, [&](auto tag) {
+    constexpr int M = decltype(tag)::value;
+    torque_kernel<M><<<grid, 128, 0, s>>>(Q, c->partial(), c->g, c->T, c->p.gm_star, ph.xp, ph.yp, ph.eps2p);
+  });
+  torque_finish_kernel<<<1, 256, 0, s>>>(c->partial(), nblocks, ph.xp, ph.yp, out);
+  c->launches += 2;
+  CUDA_TRY(c, cudaGetLastError());
+  double res[3] = {0, 0, 0};
+  CUDA_TRY(c, cudaMemcpyAsync(res, out, sizeof res, cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  *gamma_z = res[0];
   return DG_OK;
 }
 

@@ -31,8 +31,12 @@ enum : int {          // KIND: what the epilogue of the stage does
   K_MID   = 2,        // a u^n + b (u + dt N)
   K_LAST  = 3,        // K_MID + fused CFL wave-speed reduction
   K_LASTD = 4,        // K_LAST + wave-killing relaxation
-  K_COUNT = 5,
+  K_GEN   = 5,        // Butcher-form sub-step: K_i = dt N(y_i) -> kout,
+                      //   out = u^n + sum_j kc[j] kin[j] + kself K_i
+  K_GENL  = 6,        // K_GEN of the last sub-step: no kout, fused CFL reduction, wave-killing if enabled
+  K_COUNT = 7,
 };
+constexpr int MAXK = 5;   // earlier slopes a Butcher sub-step can read (Cash-Karp: 5)
 enum : int { G_NONE = 0, G_STAR = 1, G_PLANET = 2 };   // GRAV: gravity source terms present
 
 struct DevTables {            // kernel-parameter (constant bank) copy of the tables
@@ -67,6 +71,13 @@ struct StageArgs {
   double a, b, dt;            // out = a u^n + b u^(s-1) + beta N; beta = b dt is folded into T and ph
   double damp_r0, damp_inv_w, damp_tau0;
   int rows;
+  // K_GEN / K_GENL: earlier slopes K_j = dt N(y_j) with their Butcher coefficients, this sub-step's own
+  // coefficient, and where to keep K_i (null: not needed again)
+  const double* kin[MAXK];
+  double kc[MAXK];
+  double kself;
+  double* kout;
+  int nk;
   Geom g;
   Phys ph;
   DevTables T;
@@ -209,10 +220,11 @@ __global__ void __launch_bounds__(M * 32, MINB)
 stage_kernel(const __grid_constant__ StageArgs A) {
   constexpr bool grav = GRAV != G_NONE;
   constexpr bool need_ri = EOS == 1 || grav;
-  constexpr bool add_u = KIND != K_RHS;
-  constexpr bool use_un = KIND >= K_MID;
-  constexpr bool do_cfl = KIND >= K_LAST;
-  constexpr bool do_damp = KIND == K_LASTD;
+  constexpr bool gen = KIND == K_GEN || KIND == K_GENL;
+  constexpr bool add_u = KIND != K_RHS && !gen;
+  constexpr bool use_un = KIND == K_MID || KIND == K_LAST || KIND == K_LASTD;
+  constexpr bool do_cfl = KIND == K_LAST || KIND == K_LASTD || KIND == K_GENL;
+  constexpr bool do_damp = KIND == K_LASTD || KIND == K_GENL;    // K_GENL: only if the zone is enabled
   constexpr int C = 4 * M * M;                   // doubles per cell
   constexpr int BS = C * 32;                     // doubles per 32-cell tile
   constexpr uint32_t TILE_BYTES = BS * sizeof(double);
@@ -286,6 +298,13 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       bulk_prefetch_l2(A.q0 + (size_t)j * row_stride + (size_t)ib * BS, TILE_BYTES);
   };
 
+  // Butcher sub-steps read u^n and the earlier slopes in the epilogue: pull the row's tiles into L2 ahead
+  auto prefetch_gen = [&](int j) {               // thread 0 only
+    const size_t off = (size_t)j * row_stride + (size_t)ib * BS;
+    bulk_prefetch_l2(A.qn + off, TILE_BYTES);
+    for (int k = 0; k < A.nk; ++k) bulk_prefetch_l2(A.kin[k] + off, TILE_BYTES);
+  };
+
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s <= NST; ++s) mbar_init(mbar + s, 1);
@@ -298,6 +317,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     tile_issue(2);
     if (use_un) un_issue(j0);
     if (do_damp) prefetch_q0(j0);
+    if (gen) prefetch_gen(j0);
   }
 
   // line r = w of the two out-of-block x-neighbours, fetched one row ahead (lanes 0..7)
@@ -345,6 +365,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       if (more) tile_issue(t + 2);               // row j+2 -> the slot row j-1 has just left
       if (use_un && j > j0) un_issue(j);         // sN is free again
       if (do_damp && more) prefetch_q0(j + 1);
+      if (gen && more) prefetch_gen(j + 1);
     }
     const double* tu = tiles + (t % NST) * BS + lane;
     const double yc = g.y0 + (j + 0.5) * g.dy;
@@ -575,7 +596,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       // wave-killing factors of this cell (row a12): out <- f0 u0 + ft out
       double f0 = 0.0, ft = 1.0;
       bool damp = false;
-      if (do_damp) {
+      if (do_damp && (KIND != K_GENL || A.damp_r0 > 0.0)) {
         const double rc = sqrt(xc * xc + yc * yc);
         if (rc > A.damp_r0) {
           const double s = (rc - A.damp_r0) * A.damp_inv_w;
@@ -590,8 +611,9 @@ stage_kernel(const __grid_constant__ StageArgs A) {
         }
       }
       // modal update in nodal form + RK combination (rows a8, a9) and store
-      double* __restrict__ qo = A.qout + j * row_stride + (size_t)ib * BS + lane;
-      const double* __restrict__ q0 = A.q0 + j * row_stride + (size_t)ib * BS + lane;
+      const size_t cell_off = j * row_stride + (size_t)ib * BS + lane;
+      double* __restrict__ qo = A.qout + cell_off;
+      const double* __restrict__ q0 = A.q0 + cell_off;
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
         double avg = 0.0;
@@ -600,6 +622,13 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           const int e = ((v * M + rr) * M + q) * 32;
           double out = sN[e + lane] + acc[v][rr];
           out = fma(T.lym[rr], HS[v], fma(-T.lyp[rr], HN[v], out));
+          if (gen) {                               // out is K_i = dt N(y_i) here
+            const double K = out;
+            if (KIND == K_GEN && A.kout && valid) A.kout[cell_off + e] = K;
+            out = __ldg(A.qn + cell_off + e);
+            for (int k = 0; k < A.nk; ++k) out = fma(A.kc[k], __ldg(A.kin[k] + cell_off + e), out);
+            out = fma(A.kself, K, out);
+          }
           if (do_damp && damp) out = fma(f0, __ldg(q0 + e), ft * out);
           if (valid) qo[e] = out;
           if (do_cfl) avg = fma(T.w[rr], out, avg);

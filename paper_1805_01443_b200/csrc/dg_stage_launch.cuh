@@ -1,5 +1,5 @@
 // Launch dispatch of the stage kernel for one DG order M: one translation unit per order
-// (dg_stage_m1.cu ... dg_stage_m5.cu) so that the 25 variants per order compile in parallel.
+// (dg_stage_m1.cu ... dg_stage_m5.cu) so that the 35 variants per order compile in parallel.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -38,7 +38,9 @@ cudaError_t launch_stage_kind(const StageArgs& A, int kind, dim3 grid, cudaStrea
     case K_FIRST: return launch_stage_variant<M, EOS, GRAV, K_FIRST>(A, grid, s);
     case K_MID:   return launch_stage_variant<M, EOS, GRAV, K_MID>(A, grid, s);
     case K_LAST:  return launch_stage_variant<M, EOS, GRAV, K_LAST>(A, grid, s);
-    default:      return launch_stage_variant<M, EOS, GRAV, K_LASTD>(A, grid, s);
+    case K_LASTD: return launch_stage_variant<M, EOS, GRAV, K_LASTD>(A, grid, s);
+    case K_GEN:   return launch_stage_variant<M, EOS, GRAV, K_GEN>(A, grid, s);
+    default:      return launch_stage_variant<M, EOS, GRAV, K_GENL>(A, grid, s);
   }
 }
 

@@ -103,4 +103,80 @@ inline void build_host_tables(int m, HostTables* T) {
   }
 }
 
+// Tables of the positivity limiter (Zhang & Shu 2010): the Gauss-Lobatto rule with
+// the fewest points that is exact for degree N_p = m-1 (2 nh - 3 >= N_p), nodes in closed form
+// (nh = 2: +-1; 3: 0, +-1; 4: +-1, +-1/sqrt 5), its first weight normalised to sum 1,
+// w_1 = 1/(nh (nh-1)) (the factor of PAPER.md:131), and the interpolation Lh[k][r] = l_r(xh_k) from
+// the Gauss nodes to the Lobatto nodes, l_r(x) = sum_a P[r][a] phi_a(x).
+struct HostLimTables {
+  int nh;
+  double xh[4];
+  double w1;
+  double Lh[4][MAXM];
+};
+
+inline void build_limiter_tables(int m, HostLimTables* L) {
+  const int nh = m <= 2 ? 2 : (m <= 4 ? 3 : 4);
+  long double xh[4];
+  if (nh == 2) { xh[0] = -1; xh[1] = 1; }
+  else if (nh == 3) { xh[0] = -1; xh[1] = 0; xh[2] = 1; }
+  else { const long double a = 1.0L / sqrtl(5.0L); xh[0] = -1; xh[1] = -a; xh[2] = a; xh[3] = 1; }
+  long double x[MAXM], w[MAXM];
+  gauss_legendre_closed(m, x, w);
+  L->nh = nh;
+  L->w1 = 1.0 / (double)(nh * (nh - 1));
+  for (int k = 0; k < nh; ++k) {
+    L->xh[k] = (double)xh[k];
+    for (int r = 0; r < m; ++r) {
+      long double s = 0;
+      for (int a = 0; a < m; ++a)
+        s += 0.5L * w[r] * (2.0L * a + 1.0L) * legendre_closed(a, x[r]) * legendre_closed(a, xh[k]);
+      L->Lh[k][r] = (double)s;
+    }
+  }
+}
+
+// Explicit Runge-Kutta schemes in Butcher form (Appendix A), coefficients typed from
+// the paper: rk 4 = Table 1 (five-stage fourth-order SSP scheme), rk 5 = Table 2
+// (Cash & Karp).  Table 1's printed b row sums to 1 - 8.8e-11 (14 digits): b is
+// divided by its sum so that the scheme is exactly consistent (reading G20).
+struct ButcherTableau { int s; double a[6][6], b[6], c[6]; };
+
+inline bool butcher_tableau(int rk, ButcherTableau* B) {
+  *B = ButcherTableau{};
+  if (rk == 4) {
+    static const double A54[5][5] = {
+        {0, 0, 0, 0, 0},
+        {0.39175222700392, 0, 0, 0, 0},
+        {0.21766909633821, 0.36841059262959, 0, 0, 0},
+        {0.08269208670950, 0.13995850206999, 0.25189177424738, 0, 0},
+        {0.06796628370320, 0.11503469844438, 0.20703489864929, 0.54497475021237, 0}};
+    static const double b54[5] = {0.14681187618661, 0.24848290924556, 0.10425883036650, 0.27443890091960,
+                                  0.22600748319395};
+    static const double c54[5] = {0, 0.39175222700392, 0.58607968896779, 0.47454236302687, 0.93501063100924};
+    B->s = 5;
+    double sum = 0.0;
+    for (int i = 0; i < 5; ++i) sum += b54[i];
+    for (int i = 0; i < 5; ++i) {
+      B->b[i] = b54[i] / sum;
+      B->c[i] = c54[i];
+      for (int j = 0; j < 5; ++j) B->a[i][j] = A54[i][j];
+    }
+    return true;
+  }
+  if (rk == 5) {
+    B->s = 6;
+    B->c[1] = 1.0 / 5; B->c[2] = 3.0 / 10; B->c[3] = 3.0 / 5; B->c[4] = 1.0; B->c[5] = 7.0 / 8;
+    B->a[1][0] = 1.0 / 5;
+    B->a[2][0] = 3.0 / 40; B->a[2][1] = 9.0 / 40;
+    B->a[3][0] = 3.0 / 10; B->a[3][1] = -9.0 / 10; B->a[3][2] = 6.0 / 5;
+    B->a[4][0] = -11.0 / 54; B->a[4][1] = 5.0 / 2; B->a[4][2] = -70.0 / 27; B->a[4][3] = 35.0 / 27;
+    B->a[5][0] = 1631.0 / 55296; B->a[5][1] = 175.0 / 512; B->a[5][2] = 575.0 / 13824;
+    B->a[5][3] = 44275.0 / 110592; B->a[5][4] = 253.0 / 4096;
+    B->b[0] = 37.0 / 378; B->b[2] = 250.0 / 621; B->b[3] = 125.0 / 594; B->b[5] = 512.0 / 1771;
+    return true;
+  }
+  return false;
+}
+
 }  // namespace dg

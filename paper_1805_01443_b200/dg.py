@@ -15,6 +15,7 @@ EXPORTS = [
     "dg_get_state_host", "dg_rhs", "dg_cfl_dt", "dg_step", "dg_step_debug", "dg_run_host",
     "dg_time", "dg_set_time", "dg_launch_count", "dg_set_tuning", "dg_stage_timing",
     "dg_stage_time_ms", "dg_stage_times_ms", "dg_probe_fp64_peak", "dg_last_error", "dg_destroy",
+    "dg_rk_stages", "dg_limit", "dg_torque",
 ]
 
 
@@ -33,6 +34,7 @@ class DGParams(C.Structure):
         ("q_planet", C.c_double), ("r_planet", C.c_double), ("eps_planet", C.c_double),
         ("omega_planet", C.c_double), ("phase0", C.c_double),
         ("damp_r0", C.c_double), ("damp_r1", C.c_double), ("t0", C.c_double),
+        ("limiter", C.c_int32), ("lim_eps", C.c_double),
     ]
 
 
@@ -76,6 +78,7 @@ def load_library(path: str | None = None):
         "dg_probe_fp64_peak": (i, [vp, C.POINTER(d)]),
         "dg_last_error": (C.c_char_p, [vp]),
         "dg_destroy": (None, [vp]),
+        "dg_rk_stages": (i, [i]), "dg_limit": (i, [vp]), "dg_torque": (i, [vp, d, C.POINTER(d)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -174,10 +177,18 @@ class DG:
         self._chk(self.L.dg_step(self._h, float(dt)), "dg_step")
 
     def step_debug(self, dt: float, out=None):
-        rk = int(self.params["rk"])
+        rk = int(self.L.dg_rk_stages(int(self.params["rk"])))
         out = self.new_device_state((rk,)) if out is None else out
         self._chk(self.L.dg_step_debug(self._h, float(dt), self._dev(out, rk * self.ncoef)), "dg_step_debug")
         return out
+
+    def limit(self):
+        self._chk(self.L.dg_limit(self._h), "dg_limit")
+
+    def torque(self, t: float) -> float:
+        g = C.c_double()
+        self._chk(self.L.dg_torque(self._h, float(t), C.byref(g)), "dg_torque")
+        return g.value
 
     def run_host(self, U_in, nsteps: int, cfl: float, U_out):
         self._chk(self.L.dg_run_host(self._h, self._host(U_in), int(nsteps), float(cfl),

@@ -61,9 +61,15 @@ def test_workspace_sizing_and_validation(lib):
     nd = lib.dg_workspace_bytes(C.byref(params_struct(pd)))
     padded = 33 * 64 * 4 * 9 * 8                        # x padded to whole 32-cell blocks
     assert nd >= 4 * padded                             # + snapshot of the initial state (bc 2 / damping)
-    for bad in (dict(order=0), dict(order=6), dict(rk=4), dict(bc=3), dict(eos=2), dict(nx=0),
+    for bad in (dict(order=0), dict(order=6), dict(rk=6), dict(rk=1), dict(limiter=2), dict(limiter=1, lim_eps=0.0), dict(bc=3), dict(eos=2), dict(nx=0),
                 dict(x1=p["x0"]), dict(gamma=1.0), dict(eos=1), dict(damp_r0=1.0, damp_r1=0.5)):
         assert lib.dg_workspace_bytes(C.byref(params_struct(dict(p, **bad)))) == 0, bad
+    # Butcher-form schemes keep their slopes K_j: rk 4 needs 4 more state buffers, rk 5 needs 5
+    for rk, extra in ((4, 4), (5, 5)):
+        nk = lib.dg_workspace_bytes(C.byref(params_struct(dict(p, rk=rk))))
+        assert (3 + extra) * state <= nk < (3 + extra) * state + 4096
+        assert lib.dg_rk_stages(rk) == extra + 1
+    assert lib.dg_rk_stages(2) == 2 and lib.dg_rk_stages(3) == 3 and lib.dg_rk_stages(7) == -1
     assert lib.dg_workspace_bytes(None) == 0
     h = C.c_void_p()
     assert lib.dg_init(C.byref(params_struct(p)), None, n, None, C.byref(h)) == -1

@@ -253,3 +253,142 @@ def test_full_size_headline_config(DG, planet):
     ref.step(dt)
     g.step(dt)
     assert rel_err(g.get_state().cpu().numpy(), ref.get_state()) < TOL_STAGE
+
+
+# ------------------------------------------------------------------------------------------------
+# Butcher-form RK (NEXT-2), positivity limiter (NEXT-1), torque (NEXT-3)
+NEXT_CASES = [
+    dict(nx=37, ny=9, m=2, eos=0, bc=0, gravity=False),
+    dict(nx=70, ny=11, m=3, eos=0, bc=1, gravity=True),
+    dict(nx=33, ny=7, m=4, eos=1, bc=2, gravity=True),
+    dict(nx=64, ny=40, m=5, eos=1, bc=2, gravity=True),
+    dict(nx=40, ny=6, m=5, eos=0, bc=0, gravity=False),
+    dict(nx=5, ny=3, m=1, eos=0, bc=0, gravity=False),
+]
+
+
+@pytest.mark.parametrize("rk", [4, 5])
+@pytest.mark.parametrize("case", NEXT_CASES, ids=_id)
+def test_butcher_rk_stage_parity(DG, case, rk):
+    """rk 4 (Table 1) and rk 5 (Cash-Karp, Table 2): every sub-step
+    result y_2..y_s, u^{n+1} within 1e-12, debug path and fused production path."""
+    p, U = _make(case, rk=rk, seed=5)
+    if case["eos"] == 1:
+        p["damp_r0"], p["damp_r1"] = 0.6, 1.2
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    g = DG(p)
+    g.set_tuning(1, 4)
+    g.set_state(dev(U))
+    dt = ref.cfl_dt(0.2)
+    st_ref = ref.step_debug(dt)
+    st = g.step_debug(dt).cpu().numpy()
+    assert st.shape[0] == oracle.rk_stages(rk) == (5 if rk == 4 else 6)
+    for s in range(st.shape[0]):
+        assert rel_err(st[s], st_ref[s]) < TOL_STAGE, f"sub-step {s + 1}"
+    assert rel_err(g.get_state().cpu().numpy(), ref.get_state()) < TOL_STAGE
+    g2 = DG(p)
+    g2.set_state(dev(U))
+    g2.step(dt)
+    assert rel_err(g2.get_state().cpu().numpy(), ref.get_state()) < TOL_STAGE
+    assert abs(g2.cfl_dt(0.2) / ref.cfl_dt(0.2) - 1.0) < 1e-12       # reduction fused in the last sub-step
+    assert abs(g2.time - ref.time) < 1e-15
+
+
+def _negative_spots(U, seed, frac=0.15):
+    """Push the density (and, through the energy, the pressure) below zero inside a seeded subset of
+    cells by inflating their non-constant modes: the cells the limiter has to act on."""
+    rng = np.random.default_rng(seed)
+    U = U.copy()
+    ny, nx = U.shape[:2]
+    hit = rng.random((ny, nx)) < frac
+    m = U.shape[-1]
+    if m > 1:
+        amp = rng.uniform(0.5, 3.0, size=(ny, nx))
+        kind = rng.integers(0, 3, size=(ny, nx))
+        for v, k in ((0, 0), (3, 1), (1, 2)):
+            sel = hit & (kind == k)
+            bump = rng.standard_normal(U[sel][:, v].shape) * amp[sel][:, None, None] * abs(U[..., v, 0, 0]).mean()
+            bump[:, 0, 0] = 0.0
+            U[sel, v] += bump
+    return U, hit
+
+
+@pytest.mark.parametrize("case", NEXT_CASES, ids=_id)
+def test_limiter_parity(DG, case):
+    """dg_limit against the oracle's limiter on a state with seeded inadmissible cells: every
+    coefficient within 1e-12, averages untouched, untouched cells bitwise unchanged."""
+    p, U = _make(case, seed=6)
+    U, hit = _negative_spots(U, seed=60)
+    p = dict(p, limiter=1, lim_eps=1e-9)
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    ref.limit()
+    out_ref = ref.get_state()
+    g = DG(p)
+    g.set_tuning(1, 4)
+    g.set_state(dev(U))
+    before = g.get_state().cpu().numpy()
+    g.limit()
+    out = g.get_state().cpu().numpy()
+    assert rel_err(out, out_ref) < TOL_STAGE
+    changed_ref = np.abs(out_ref - U).max(axis=(2, 3, 4)) > 0
+    if case["m"] > 1:
+        assert changed_ref.sum() >= 3                     # the test exercises the limiter
+    same = ~changed_ref
+    np.testing.assert_array_equal(out[same], before[same])
+    np.testing.assert_allclose(out[..., 0, 0], U[..., 0, 0], rtol=1e-14)
+
+
+@pytest.mark.parametrize("rk", [2, 3, 5])
+@pytest.mark.parametrize("case", NEXT_CASES[:5], ids=_id)
+def test_limited_step_parity(DG, case, rk):
+    """A full step with the limiter after every sub-step, from a state the limiter has
+    just made admissible but which the step drives negative again in places; fused tail
+    (limiter + wave-killing + CFL in one pass) against the debug path and the oracle."""
+    p, U = _make(case, rk=rk, seed=7)
+    U, hit = _negative_spots(U, seed=70, frac=0.1)
+    p = dict(p, limiter=1, lim_eps=1e-9)
+    if case["eos"] == 1:
+        p["damp_r0"], p["damp_r1"] = 0.6, 1.2
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    ref.limit()
+    U1 = ref.get_state()
+    ref.set_state(U1)
+    g = DG(p)
+    g.set_state(dev(U1))
+    dt_ref = ref.cfl_dt(0.2)
+    assert abs(g.cfl_dt(0.2) / dt_ref - 1.0) < 1e-13       # includes the w_1/2 factor (PAPER.md:131)
+    dt = 0.5 * dt_ref
+    st_ref = ref.step_debug(dt)
+    st = g.step_debug(dt).cpu().numpy()
+    for s in range(st.shape[0]):
+        assert np.isfinite(st_ref[s]).all()
+        assert rel_err(st[s], st_ref[s]) < 2 * TOL_STAGE, f"sub-step {s + 1}"
+    assert rel_err(g.get_state().cpu().numpy(), ref.get_state()) < 2 * TOL_STAGE
+    g2 = DG(p)
+    g2.set_state(dev(U1))
+    g2.step(dt)
+    assert rel_err(g2.get_state().cpu().numpy(), ref.get_state()) < 2 * TOL_STAGE
+    assert abs(g2.cfl_dt(0.2) / ref.cfl_dt(0.2) - 1.0) < 1e-12
+
+
+@pytest.mark.parametrize("case", NEXT_CASES[1:4], ids=_id)
+def test_torque_parity(DG, case):
+    p, U = _make(case, seed=8)
+    ref = oracle.RefDG(p)
+    ref.set_state(U)
+    g = DG(p)
+    g.set_state(dev(U))
+    for t in (0.0, 1.7):
+        gr = ref.torque(t)
+        scale = np.abs(U[..., 0, 0, 0]).sum() * (p["x1"] - p["x0"]) / p["nx"] * (p["y1"] - p["y0"]) / p["ny"]
+        assert abs(g.torque(t) - gr) < 1e-12 * max(abs(gr), scale)
+
+
+def test_100_steps_butcher_limited_disc(DG):
+    """configs[3] shape at 48^2, order 4, Cash-Karp, limiter on: 100 free-running steps within 1e-10."""
+    p, U = W.disc(48, 4, planet=True, noise=1e-4, rk=5)
+    p = dict(p, limiter=1)
+    assert _run_100(DG, p, U) < TOL_100
