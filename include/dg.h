@@ -112,8 +112,8 @@ int dg_rk_stages(int rk);
 
 /* Apply the positivity-preserving limiter (Zhang & Shu 2010) to the current state, in
  * place, with floor lim_eps -- whether or not params.limiter is set (e.g. on a freshly projected initial
- * state).  Cell averages are unchanged.  Per cell K, with S_K = (Gauss_m x Lobatto_nh) U (Lobatto_nh x Gauss_m),
- * nh the smallest Gauss-Lobatto rule exact for degree N_p:
+ * state).  Cell averages are unchanged.  Per cell K, with S_K = (Gauss_m x Lobatto_nh) U (Lobatto_nh x Gauss_m)
+ * U (Gauss_m x Gauss_m, the volume quadrature points), nh the smallest Gauss-Lobatto rule exact for degree N_p:
  *   theta1 = min(1, (rho_bar - eps)/(rho_bar - min_S rho)) scales the density's non-constant part; then
  *   (eos 0) theta2 = min over the points of S_K with p < eps of the parameter t at which the segment
  *   u_bar + t (u(x) - u_bar) meets p = eps, and scales all four variables' non-constant parts. */

@@ -365,7 +365,9 @@ void damp(ref_ctx* c, double dt) {
 /* ---- C12: positivity-preserving limiter (Zhang & Shu 2010, step (iii)(d) PAPER.md:150) ----
  * Point set S_K of a rectangle (Zhang & Shu 2010, their S_ij): (Gauss_m in x) x (Lobatto_nh in y) united
  * with (Lobatto_nh in x) x (Gauss_m in y), nh the smallest Gauss-Lobatto rule exact for degree
- * N_p: 2 nh - 3 >= N_p. */
+ * N_p: 2 nh - 3 >= N_p; plus the m x m tensor Gauss points at which the volume integral of Eq.(3)
+ * samples the flux (Zhang & Shu's remark that the points used by the scheme's quadratures belong to
+ * the set; reading L2), so that every state the scheme evaluates a flux at is admissible. */
 
 void build_lobatto(int m, LimTables* LT) {
   const int Np = m - 1;
@@ -423,6 +425,8 @@ int limiter_points(const Tables& T, const LimTables& LT, LimPoint* pts) {
       pts[n].px = T.B[q];  pts[n].py = LT.Bh[k]; ++n;      /* Gauss in x, Lobatto in y */
       pts[n].px = LT.Bh[k]; pts[n].py = T.B[q];  ++n;      /* Lobatto in x, Gauss in y */
     }
+  for (int q = 0; q < T.m; ++q)
+    for (int r = 0; r < T.m; ++r) { pts[n].px = T.B[q]; pts[n].py = T.B[r]; ++n; }   /* volume Gauss points */
   return n;
 }
 
@@ -430,7 +434,7 @@ void limit_cell(const ref_params& p, const Tables& T, const LimTables& LT, doubl
   const int m = T.m;
   double th1 = 1.0, th2 = 1.0;
   if (m > 1) {
-    LimPoint pts[2 * MAXM * 4];
+    LimPoint pts[2 * MAXM * 4 + MAXM * MAXM];
     const int npts = limiter_points(T, LT, pts);
     double ubar[NV];
     for (int v = 0; v < NV; ++v) ubar[v] = u[v * m * m];          /* mode (0,0) = cell average */

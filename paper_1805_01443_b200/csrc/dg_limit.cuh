@@ -5,7 +5,8 @@
 //   torque_kernel  specific torque on the planet, Eq.(6)
 //
 // Limiter in nodal form.  The points of Zhang & Shu's set S_K are (Gauss_m in x) x (Lobatto_nh in y)
-// and (Lobatto_nh in x) x (Gauss_m in y).  Thread (warp w, lane) holds column xi_w of its cell in
+// and (Lobatto_nh in x) x (Gauss_m in y), plus the m x m Gauss points of the volume integral (the
+// nodal values themselves: DESIGN.md reading L2).  Thread (warp w, lane) holds column xi_w of its cell in
 // registers and reads line eta_w of the same cell from the shared-memory copy of the tile, so the
 // values at its 2 nh points are two 1-D interpolations Lh[k][.] (Gauss nodes -> Lobatto nodes).
 // Scaling the non-constant modes by theta is, on nodal values, u <- ubar + theta (u - ubar).
@@ -151,8 +152,10 @@ limit_kernel(const __grid_constant__ LimitArgs A) {
       for (int q = 0; q < M; ++q) s += sAvg[(v * M + q) * 32 + lane];
       ub[v] = s;
     }
-    // step 1: density minimum over this thread's 2 nh points
+    // step 1: density minimum over this thread's 2 nh points and its column's m nodes
     double rmin = ub[0];
+#pragma unroll
+    for (int r = 0; r < M; ++r) rmin = fmin(rmin, uc[0][r]);
     for (int k = 0; k < LT.nh; ++k) {
       double a = 0.0, b = 0.0;
 #pragma unroll
@@ -191,6 +194,12 @@ limit_kernel(const __grid_constant__ LimitArgs A) {
           const double pr = A.ph.gm1 * (s[3] - 0.5 * (s[1] * s[1] + s[2] * s[2]) / s[0]);
           if (pr < eps_p) tmin = fmin(tmin, segment_root(ub, s, e1));
         }
+      }
+#pragma unroll
+      for (int r = 0; r < M; ++r) {               // the column's own nodes
+        double s[4] = {fma(th1, uc[0][r] - ub[0], ub[0]), uc[1][r], uc[2][r], uc[3][r]};
+        const double pr = A.ph.gm1 * (s[3] - 0.5 * (s[1] * s[1] + s[2] * s[2]) / s[0]);
+        if (pr < eps_p) tmin = fmin(tmin, segment_root(ub, s, e1));
       }
       sT[w * 32 + lane] = tmin;
       __syncthreads();

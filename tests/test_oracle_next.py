@@ -132,7 +132,8 @@ def _limiter_point_values(m, u):
     xh, _ = oracle.lobatto(m)
     a = _cell_values(u, xg, xh).reshape(4, -1)            # Gauss in x, Lobatto in y
     b = _cell_values(u, xh, xg).reshape(4, -1)            # Lobatto in x, Gauss in y
-    return np.concatenate([a, b], axis=1)
+    c = _cell_values(u, xg, xg).reshape(4, -1)            # the volume quadrature's tensor Gauss points
+    return np.concatenate([a, b, c], axis=1)
 
 
 @pytest.mark.parametrize("m", [2, 3, 4, 5])
