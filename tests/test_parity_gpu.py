@@ -371,7 +371,9 @@ def test_limited_step_parity(DG, case, rk):
     g2.set_state(dev(U1))
     g2.step(dt)
     assert rel_err(g2.get_state().cpu().numpy(), ref.get_state()) < 2 * TOL_STAGE
-    assert abs(g2.cfl_dt(0.2) / ref.cfl_dt(0.2) - 1.0) < 1e-12
+    # the seeded spots leave cells whose average density is ~1e-3 of the maximum: v = m / rho_bar there
+    # amplifies the 1e-12-of-max state difference, so the fused reduction is compared at 1e-9
+    assert abs(g2.cfl_dt(0.2) / ref.cfl_dt(0.2) - 1.0) < 1e-9
 
 
 @pytest.mark.parametrize("case", NEXT_CASES[1:4], ids=_id)
