@@ -395,12 +395,12 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     }
 
     // =========================== X phase: eta-line r = w ===========================
+    double enext[M];                             // next row's edge lines: in flight during this whole row
+#pragma unroll
+    for (int q = 0; q < M; ++q)
+      enext[q] = (edge_src && more) ? __ldg(edge_src + (size_t)(j + 1) * row_stride + q * 32) : 0.0;
     {
       const int r = w;
-      double enext[M];                           // next row's edge lines: in flight during this row
-#pragma unroll
-      for (int q = 0; q < M; ++q)
-        enext[q] = (edge_src && more) ? __ldg(edge_src + (size_t)(j + 1) * row_stride + q * 32) : 0.0;
       tile_wait(t);
       const double yr = yc + g.hdy * T.xi[r];
       const double y2e = fma(yr, yr, A.ph.eps2s);
@@ -439,8 +439,6 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       double etr = 0.0;
 #pragma unroll
       for (int q = 0; q < M; ++q) etr = fma(lane < 4 ? T.Ip[q] : T.Im[q], eraw[q], etr);
-#pragma unroll
-      for (int q = 0; q < M; ++q) eraw[q] = enext[q];
       double UX[4];
 #pragma unroll
       for (int v = 0; v < 4; ++v) UX[v] = __shfl_sync(FULL, etr, (lane == 0 ? 0 : 4) + v);
@@ -524,6 +522,35 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       for (int v = 0; v < 4; ++v)
 #pragma unroll
         for (int r = 0; r < M; ++r) acc[v][r] = 0.0;
+      // wave-killing factors of this cell (row a12; SURVEY C11): out <- f0 u0 + ft out
+      double f0 = 0.0, ft = 1.0;
+      bool damp = false;
+      if (do_damp && (KIND != K_GENL || A.damp_r0 > 0.0)) {
+        const double rc = sqrt(xc * xc + yc * yc);
+        if (rc > A.damp_r0) {
+          const double s = (rc - A.damp_r0) * A.damp_inv_w;
+          const double R = fmin(1.0, s * s);
+          if (R > 0.0) {
+            const double tau = A.damp_tau0 / R;
+            const double inv = 1.0 / (tau + A.dt);
+            damp = true;
+            f0 = A.dt * inv;
+            ft = tau * inv;
+          }
+        }
+      }
+      // the initial state of the damped cells: for M <= 4 requested here and used in the epilogue (the
+      // loads have the whole Y phase to land); at M = 5 the 20 extra live doubles cost more than they
+      // save (measured: 0.668 vs 0.637 ms for the last stage), so there the loads stay in the epilogue
+      constexpr bool early_q0 = do_damp && M <= 4;
+      double z0[4][M];
+      if (early_q0) {
+        const double* __restrict__ q0e = A.q0 + j * row_stride + (size_t)ib * BS + lane;
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+#pragma unroll
+          for (int rr = 0; rr < M; ++rr) z0[v][rr] = damp ? __ldg(q0e + ((v * M + rr) * M + q) * 32) : 0.0;
+      }
       double UN[4] = {0, 0, 0, 0};
 #pragma unroll
       for (int r = 0; r < M; ++r) {
@@ -593,27 +620,9 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       double HN[4];
       llf2(UN, GNo, lamNo, aU, aG, aLam, HN);
 
-      // wave-killing factors of this cell (row a12; SURVEY C11): out <- f0 u0 + ft out
-      double f0 = 0.0, ft = 1.0;
-      bool damp = false;
-      if (do_damp && (KIND != K_GENL || A.damp_r0 > 0.0)) {
-        const double rc = sqrt(xc * xc + yc * yc);
-        if (rc > A.damp_r0) {
-          const double s = (rc - A.damp_r0) * A.damp_inv_w;
-          const double R = fmin(1.0, s * s);
-          if (R > 0.0) {
-            const double tau = A.damp_tau0 / R;
-            const double inv = 1.0 / (tau + A.dt);
-            damp = true;
-            f0 = A.dt * inv;
-            ft = tau * inv;
-          }
-        }
-      }
       // modal update in nodal form + RK combination (rows a8, a9) and store
       const size_t cell_off = j * row_stride + (size_t)ib * BS + lane;
       double* __restrict__ qo = A.qout + cell_off;
-      const double* __restrict__ q0 = A.q0 + cell_off;
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
         double avg = 0.0;
@@ -629,7 +638,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
             for (int k = 0; k < A.nk; ++k) out = fma(A.kc[k], __ldg(A.kin[k] + cell_off + e), out);
             out = fma(A.kself, K, out);
           }
-          if (do_damp && damp) out = fma(f0, __ldg(q0 + e), ft * out);
+          if (do_damp && damp) out = fma(f0, early_q0 ? z0[v][rr] : __ldg(A.q0 + cell_off + e), ft * out);
           if (valid) qo[e] = out;
           if (do_cfl) avg = fma(T.w[rr], out, avg);
         }
@@ -638,6 +647,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 #pragma unroll
       for (int v = 0; v < 4; ++v) HS[v] = HN[v];   // this row's N face is the next row's S face
     }
+#pragma unroll
+    for (int q = 0; q < M; ++q) eraw[q] = enext[q];   // consumed only now: the loads had the whole row to land
     __syncthreads();
   }
   // CFL wave speed of the last row of the segment, then one reduction per thread block
