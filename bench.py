@@ -4,6 +4,7 @@
     python bench.py [--gpus N] [--steps K] [--warmup W]           # this repo's CUDA path
     python bench.py --impl reference [--steps K] [--warmup W]     # the CPU oracle, as it stands
     python bench.py --sweep                                       # configs[4]: orders x grids table
+    python bench.py --variants                                    # RK(5,4), Cash-Karp, limiter, torque
 
 A *step* is one full time step of the hot path on BASELINE configs[3] (planet-disc, 1024^2 cells,
 order 5, SSP-RK3): dg_cfl_dt (row a10 of SURVEY.md 8(a); its reduction rides on the previous last
@@ -389,6 +390,84 @@ def run_sweep(args):
             torch.cuda.empty_cache()
 
 
+def step_arrays(p: dict, f_damp: float) -> float:
+    """Algorithmic state-sized arrays one time step moves (reads + writes), for any scheme / limiter:
+    SSP forms: 2 + 3 (rk-1); Butcher form sub-step i (0-based, s sub-steps): reads y_i, u^n (one array when
+    i = 0) and the earlier slopes with non-zero coefficient, writes K_i (not the last) and y_{i+1};
+    limiter: one more read per sub-step (writes only the cells it changes); wave-killing: f_damp."""
+    rk = p["rk"]
+    if rk <= 3:
+        arrays, sub = 2 + 3 * (rk - 1), rk
+    else:
+        nz = {4: [0, 1, 2, 3, 4], 5: [0, 1, 2, 3, 4, 3]}[rk]     # non-zero a_{i+1,j}, j < i (last row: b)
+        sub = len(nz)
+        arrays = 0
+        for i in range(sub):
+            arrays += (1 if i == 0 else 2) + nz[i] + (1 if i + 1 < sub else 0) + 1
+    if p.get("limiter"):
+        arrays += sub
+    return arrays + f_damp
+
+
+def run_variants(args):
+    """SURVEY.md 8(f) rows on the bench workload's shape: one JSON line per variant (1 GPU)."""
+    import numpy as np
+    import torch
+    from paper_1805_01443_b200 import DG, workloads as W
+    from paper_1805_01443_b200.build import build
+    build()
+    peak, peak_src = load_peaks()
+    n, m = args.n, args.order
+    for name, over in (("ssp33 (bench)", {}), ("ssp33 + limiter", {"limiter": 1}),
+                       ("rk4: SSP-RK(5,4), paper Table 1", {"rk": 4}), ("rk5: Cash-Karp, paper Table 2", {"rk": 5}),
+                       ("rk5 + limiter", {"rk": 5, "limiter": 1})):
+        p, U = W.disc(n, m, planet=True, noise=1e-4)
+        p.update(over)
+        g = DG(p)
+        g.set_state(torch.from_numpy(U).cuda())
+        del U
+        for _ in range(3):
+            g.step(g.cfl_dt(CFL))
+        torch.cuda.synchronize()
+        steps = args.sweep_steps
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = g.launch_count
+        ev0.record()
+        for _ in range(steps):
+            g.step(g.cfl_dt(CFL))
+        ev1.record()
+        torch.cuda.synchronize()
+        ms = ev0.elapsed_time(ev1) / steps
+        _, acct = stage_bytes_per_launch(dict(p, rk=3))
+        arrays = step_arrays(p, acct["damping_zone_fraction"])
+        sub = {2: 2, 3: 3, 4: 5, 5: 6}[p["rk"]]
+        gbs = arrays * acct["state_bytes"] / (ms * 1e-3) / 1e9
+        line = {"variant": name, "n": n, "order": m, "rk": p["rk"], "limiter": p["limiter"], "sub_steps": sub,
+                "steps": steps, "ms_per_step": ms, "ms_per_sub_step": ms / sub,
+                "dof_updates_per_s": W.dof_count(p) * sub / (ms * 1e-3),
+                "launches_per_step": (g.launch_count - l0) / steps,
+                "algorithmic_arrays_per_step": round(arrays, 3), "hbm_gbs": gbs, "hbm_frac": gbs / peak,
+                "peak": peak, "peak_source": peak_src}
+        if name.startswith("ssp33 (bench)"):
+            t0 = g.time
+            g.torque(t0)
+            torch.cuda.synchronize()
+            ev0.record()
+            for _ in range(20):
+                g.torque(t0)
+            ev1.record()
+            torch.cuda.synchronize()
+            tms = ev0.elapsed_time(ev1) / 20
+            tb = acct["state_bytes"] / 4
+            line["torque"] = {"ms_per_call": tms, "algorithmic_bytes": tb, "hbm_gbs": tb / (tms * 1e-3) / 1e9,
+                              "hbm_frac": tb / (tms * 1e-3) / 1e9 / peak,
+                              "note": "dg_torque: density nodes of the whole grid -> 2 kernels + one 24-byte D2H (blocking)"}
+        print(json.dumps(line), flush=True)
+        g.close()
+        del g
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -401,12 +480,16 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--variants", action="store_true")
     ap.add_argument("--sweep-grids", default="256,512,1024,2048")
     ap.add_argument("--sweep-orders", default="1,2,3,4,5")
     ap.add_argument("--sweep-steps", type=int, default=50)
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)
+        return
+    if args.variants:
+        run_variants(args)
         return
     out = run_reference_arm(args) if args.impl == "reference" else run_cuda_arm(args)
     if out is not None:

@@ -626,6 +626,18 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
         double avg = 0.0;
+        // Butcher sub-step: u^n and the earlier slopes of this variable's column, all requested before the
+        // first use (independent loads in flight together; slots >= nk are predicated off)
+        double gb[M], gk[MAXK][M];
+        if (gen) {
+#pragma unroll
+          for (int rr = 0; rr < M; ++rr) gb[rr] = __ldg(A.qn + cell_off + ((v * M + rr) * M + q) * 32);
+#pragma unroll
+          for (int k = 0; k < MAXK; ++k)
+#pragma unroll
+            for (int rr = 0; rr < M; ++rr)
+              gk[k][rr] = k < A.nk ? __ldg(A.kin[k] + cell_off + ((v * M + rr) * M + q) * 32) : 0.0;
+        }
 #pragma unroll
         for (int rr = 0; rr < M; ++rr) {
           const int e = ((v * M + rr) * M + q) * 32;
@@ -634,8 +646,9 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           if (gen) {                               // out is K_i = dt N(y_i) here
             const double K = out;
             if (KIND == K_GEN && A.kout && valid) A.kout[cell_off + e] = K;
-            out = __ldg(A.qn + cell_off + e);
-            for (int k = 0; k < A.nk; ++k) out = fma(A.kc[k], __ldg(A.kin[k] + cell_off + e), out);
+            out = gb[rr];
+#pragma unroll
+            for (int k = 0; k < MAXK; ++k) out = fma(A.kc[k], gk[k][rr], out);   // kc = 0 beyond nk
             out = fma(A.kself, K, out);
           }
           if (do_damp && damp) out = fma(f0, early_q0 ? z0[v][rr] : __ldg(A.q0 + cell_off + e), ft * out);

@@ -17,6 +17,8 @@ PAPER.md:266-313, with the shapes BASELINE.json fixes):
 * ``disc``    -- locally isothermal Keplerian disc, optional planet and seeded
                  multiplicative noise (BASELINE cfg1..cfg4).
 * ``random_smooth`` -- seeded smooth positive random state for parity tests.
+* ``gresho``  -- Gresho vortex.
+* ``paper_disc`` -- the paper's own adiabatic planet-disc setup, PAPER.md:266-313 (NEXT-3).
 """
 from __future__ import annotations
 
@@ -144,6 +146,39 @@ def entropy_wave(n: int = 16, order: int = 3, rk: int = 3, amp: float = 0.2):
 
 def entropy_wave_exact(X, Y, t, amp: float = 0.2):
     return 1.0 + amp * np.sin(2.0 * math.pi * (X + Y - 2.0 * t) / 10.0)
+
+
+def gresho(n: int = 40, order: int = 3, rk: int = 3, gamma: float = 1.4):
+    """Gresho vortex: steady rotating flow on [0,1]^2 centred at (0.5, 0.5), rho = 1,
+    v_phi = 5r | 2-5r | 0 and the pressure that balances it, gradient-free boundaries (the
+    transmissive bc 1).  Table 1 is quoted at 40 x 40 cells, T = 3.  gamma is not
+    stated in the paper; 1.4 as in Liska & Wendroff (2003), whom the paper follows."""
+    p = make_params(nx=n, ny=n, x0=0.0, x1=1.0, y0=0.0, y1=1.0, order=order, rk=rk, bc=1, eos=0, gamma=gamma)
+    X, Y = _mesh(p)
+    rho, vx, vy, pr = gresho_exact(X, Y)
+    return p, project_nodal(p, _conservative(rho, vx, vy, pr, gamma))
+
+
+def gresho_exact(X, Y):
+    """Primitive fields of the (time-independent) Gresho vortex."""
+    dx, dy = X - 0.5, Y - 0.5
+    r = np.sqrt(dx * dx + dy * dy)
+    rs = np.maximum(r, 1e-300)
+    vphi = np.where(r < 0.2, 5.0 * r, np.where(r < 0.4, 2.0 - 5.0 * r, 0.0))
+    pr = np.where(r < 0.2, 5.0 + 12.5 * r * r,
+                  np.where(r < 0.4, 9.0 - 4.0 * math.log(0.2) + 12.5 * r * r - 20.0 * r + 4.0 * np.log(rs),
+                           3.0 + 4.0 * math.log(2.0)))
+    return np.ones_like(r), -vphi * dy / rs, vphi * dx / rs, pr
+
+
+def l1_error_percent(p: dict, U: np.ndarray, exact_nodal: np.ndarray, v: int = 0) -> float:
+    """Relative L1 error (%) of variable v by the quadrature of Eq.(5):
+    100 * sum_K sum_ij |u_h - u| w_i w_j / sum_K sum_ij |u| w_i w_j  (the 1/4 dx dy cancels)."""
+    m = p["order"]
+    _, w = _nodes_weights(m)
+    ww = w[:, None] * w[None, :]
+    uh = evaluate_nodal(p, U)[:, :, v]
+    return float(100.0 * (np.abs(uh - exact_nodal) * ww).sum() / (np.abs(exact_nodal) * ww).sum())
 
 
 # ----------------------------------------------------------------------------------------------

@@ -394,3 +394,23 @@ def test_100_steps_butcher_limited_disc(DG):
     p, U = W.disc(48, 4, planet=True, noise=1e-4, rk=5)
     p = dict(p, limiter=1)
     assert _run_100(DG, p, U) < TOL_100
+
+
+def test_gresho_table1_soft_pin_on_gpu(DG):
+    """Gresho vortex, 40 x 40, T = 3 through the CUDA path at DG2, DG3, DG4: relative L1
+    density errors fall with the order as in Table 1 (0.05 / 0.01 / 0.008 %) and stay within a factor 4
+    of it (soft pin: the paper does not state flux, CFL number or RK order of those runs)."""
+    table = {2: 0.05, 3: 0.01, 4: 0.008}
+    errs = {}
+    for m in (2, 3, 4):
+        p, U = W.gresho(40, m, rk=min(m, 3))
+        p["bc"] = 0
+        g = DG(p)
+        g.set_state(dev(U))
+        while g.time < 3.0:
+            g.step(min(g.cfl_dt(0.2), 3.0 - g.time))
+        X, _ = W._mesh(p)
+        errs[m] = W.l1_error_percent(p, g.get_state().cpu().numpy(), np.ones_like(X))
+    assert errs[2] > errs[3] > errs[4], errs
+    for m in (2, 3, 4):
+        assert table[m] / 4 < errs[m] < table[m] * 4, errs
