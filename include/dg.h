@@ -65,6 +65,9 @@ typedef struct {
                                      every RK sub-step (step (iii)(d)), and dg_cfl_dt uses the factor
                                      min(1/(2N_p+1), w_1/2) of PAPER.md:131; 0: off */
   double  lim_eps;                /* limiter floor for density and pressure (> 0 when limiter = 1; 1e-13) */
+  double  damp_in_r0, damp_in_r1; /* inner wave-killing zone of the paper's own disc: active for
+                                     r < damp_in_r0 (= r_d), full strength for r <= damp_in_r1 (= r_in < r_d);
+                                     damp_in_r0 <= 0: off */
 } dg_params;
 
 /* Bytes of DEVICE workspace dg_init needs for these parameters (0 if they are invalid). */

@@ -43,6 +43,7 @@ class RefParams(C.Structure):
         ("omega_planet", C.c_double), ("phase0", C.c_double),
         ("damp_r0", C.c_double), ("damp_r1", C.c_double), ("t0", C.c_double),
         ("limiter", C.c_int32), ("lim_eps", C.c_double),
+        ("damp_in_r0", C.c_double), ("damp_in_r1", C.c_double),
     ]
 
 

@@ -340,22 +340,32 @@ void dg_ode(void* user, double t, const double* y, double* dydt) {
   compute_rhs(static_cast<RhsClosure*>(user)->c, y, t, 7, dydt);
 }
 
-/* C11 */
+/* C11: Q <- (dt Q0 + tau Q)/(tau + dt), tau = 2 pi sqrt(r_d^3/GM)/R(r), R(r) = ((r - r_d)/(r_b - r_d))^2
+ * clamped to 1 beyond the boundary radius r_b.  Outer zone: r_d = damp_r0 < r,
+ * r_b = damp_r1; inner zone (the paper's own disc): r_d = damp_in_r0 > r, r_b = damp_in_r1. */
 void damp(ref_ctx* c, double dt) {
   const ref_params& p = c->p;
-  if (!(p.damp_r0 > 0.0)) return;
+  if (!(p.damp_r0 > 0.0) && !(p.damp_in_r0 > 0.0)) return;
   const int m = c->m;
   const double pi = 3.14159265358979323846;
   for (int j = 0; j < p.ny; ++j)
     for (int i = 0; i < p.nx; ++i) {
       const double xc = p.x0 + (i + 0.5) * c->dx, yc = p.y0 + (j + 0.5) * c->dy;
       const double r = std::sqrt(xc * xc + yc * yc);
-      if (!(r > p.damp_r0)) continue;
-      double s = (r - p.damp_r0) / (p.damp_r1 - p.damp_r0);
+      double rd, s;
+      if (p.damp_r0 > 0.0 && r > p.damp_r0) {
+        rd = p.damp_r0;
+        s = (r - p.damp_r0) / (p.damp_r1 - p.damp_r0);
+      } else if (p.damp_in_r0 > 0.0 && r < p.damp_in_r0) {
+        rd = p.damp_in_r0;
+        s = (p.damp_in_r0 - r) / (p.damp_in_r0 - p.damp_in_r1);
+      } else {
+        continue;
+      }
       double R = s * s;
       if (R > 1.0) R = 1.0;
       if (!(R > 0.0)) continue;
-      const double tau = 2.0 * pi * std::sqrt(p.damp_r0 * p.damp_r0 * p.damp_r0 / p.gm_star) / R;
+      const double tau = 2.0 * pi * std::sqrt(rd * rd * rd / p.gm_star) / R;
       double* u = c->U.data() + cell_off(c, i, j);
       const double* u0 = c->U0.data() + cell_off(c, i, j);
       for (int k = 0; k < NV * m * m; ++k) u[k] = (dt * u0[k] + tau * u[k]) / (tau + dt);
@@ -558,6 +568,7 @@ int check_params(const ref_params* p) {
   if (p->damp_r0 > 0.0 && !(p->damp_r1 > p->damp_r0 && p->gm_star > 0.0)) return -1;
   if (p->limiter != 0 && p->limiter != 1) return -1;
   if (p->limiter == 1 && !(p->lim_eps > 0.0)) return -1;
+  if (p->damp_in_r0 > 0.0 && !(p->damp_in_r1 >= 0.0 && p->damp_in_r1 < p->damp_in_r0 && p->gm_star > 0.0)) return -1;
   return 0;
 }
 

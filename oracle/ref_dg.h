@@ -38,6 +38,8 @@ typedef struct {
   int32_t limiter;           /* 1: positivity-preserving limiter (Zhang & Shu 2010) after every
                                 RK sub-step and the w_1/2 factor in the time step */
   double  lim_eps;           /* the limiter's floor for density and pressure (Zhang & Shu use 1e-13) */
+  double  damp_in_r0, damp_in_r1; /* inner wave-killing zone r < damp_in_r0 (r_d = r_in 1.15^(3/2),
+                                     boundary radius r_in = damp_in_r1); damp_in_r0 <= 0: off */
 } ref_params;
 
 /* --- the same surface as include/dg.h, prefixed ref_, host memory --- */

@@ -31,6 +31,8 @@ struct Layout {
   size_t off_q[3], off_k[MAXK], off_q0, off_btrW, off_btrE, off_btrS, off_btrN, off_partial, off_scalars, total;
 };
 
+inline bool has_damping(const dg_params& p) { return p.damp_r0 > 0.0 || p.damp_in_r0 > 0.0; }
+
 bool valid_params(const dg_params* p) {
   if (!p) return false;
   if (p->nx < 1 || p->ny < 1 || p->order < 1 || p->order > MAXM) return false;
@@ -42,6 +44,8 @@ bool valid_params(const dg_params* p) {
   if (p->eos == 0 && !(p->gamma > 1.0)) return false;
   if (p->eos == 1 && !(p->h_aspect > 0.0 && p->gm_star > 0.0)) return false;
   if (p->damp_r0 > 0.0 && !(p->damp_r1 > p->damp_r0 && p->gm_star > 0.0)) return false;
+  if (p->damp_in_r0 > 0.0 && !(p->damp_in_r1 >= 0.0 && p->damp_in_r1 < p->damp_in_r0 && p->gm_star > 0.0)) return false;
+  if (p->damp_in_r0 > 0.0 && p->damp_r0 > 0.0 && !(p->damp_in_r0 <= p->damp_r0)) return false;
   if (p->gm_star < 0.0 || p->q_planet < 0.0) return false;
   return true;
 }
@@ -52,7 +56,7 @@ Layout make_layout(const dg_params* p) {
   L.nbx = (p->nx + 31) / 32;
   L.state_doubles = (size_t)p->ny * L.nbx * 4 * L.m * L.m * 32;
   L.state_bytes = align_up(L.state_doubles * sizeof(double));
-  L.need_q0 = p->bc == 2 || p->damp_r0 > 0.0;
+  L.need_q0 = p->bc == 2 || has_damping(*p);
   L.need_btr = p->bc == 2;
   size_t off = 0;
   for (int k = 0; k < 3; ++k) { L.off_q[k] = off; off += L.state_bytes; }
@@ -153,6 +157,27 @@ Phys make_phys(const dg_ctx* c, double t, double beta = 1.0) {
   return ph;
 }
 
+// wave-killing zones of this context for a step of size dt (all off when !enable)
+DampArgs make_damp(const dg_ctx* c, double dt, bool enable = true) {
+  DampArgs D{};
+  const dg_params& p = c->p;
+  const double two_pi = 2.0 * 3.14159265358979323846;
+  D.dt = dt;
+  D.r0 = INFINITY;
+  D.on = enable && has_damping(p);
+  if (enable && p.damp_r0 > 0.0) {
+    D.r0 = p.damp_r0;
+    D.inv_w = 1.0 / (p.damp_r1 - p.damp_r0);
+    D.tau0 = two_pi * std::sqrt(p.damp_r0 * p.damp_r0 * p.damp_r0 / p.gm_star);
+  }
+  if (enable && p.damp_in_r0 > 0.0) {
+    D.in_r0 = p.damp_in_r0;
+    D.in_inv_w = 1.0 / (p.damp_in_r0 - p.damp_in_r1);
+    D.in_tau0 = two_pi * std::sqrt(p.damp_in_r0 * p.damp_in_r0 * p.damp_in_r0 / p.gm_star);
+  }
+  return D;
+}
+
 // One fused stage: qout = a*qn + b*(qprev + dt*L(qprev, t))  (kind selects the epilogue, K_* in
 // dg_kernels.cuh; K_RHS writes L itself).  The kernel computes a*qn + b*qprev + beta*L with
 // beta = b*dt folded into the derivative / lifting tables and the gravity constants here; the
@@ -178,11 +203,7 @@ int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout,
   A.btrW = c->btrW(); A.btrE = c->btrE(); A.btrS = c->btrS(); A.btrN = c->btrN();
   A.wmax = c->wmax();
   A.a = a; A.b = b; A.dt = dt;
-  A.damp_r0 = c->p.damp_r0;
-  A.damp_inv_w = c->p.damp_r0 > 0.0 ? 1.0 / (c->p.damp_r1 - c->p.damp_r0) : 0.0;
-  A.damp_tau0 = c->p.damp_r0 > 0.0
-      ? 2.0 * 3.14159265358979323846 * std::sqrt(c->p.damp_r0 * c->p.damp_r0 * c->p.damp_r0 / c->p.gm_star)
-      : 0.0;
+  A.D = make_damp(c, dt);
   A.rows = c->rows_per_cta;
   A.g = c->g;
   A.ph = make_phys(c, t, beta);
@@ -275,17 +296,16 @@ int finish_set_state(dg_ctx* c) {
 
 int launch_damp(dg_ctx* c, double* Q, double dt) {
   dim3 grid(c->L.nbx, (c->p.ny + 3) / 4);
-  const double r0 = c->p.damp_r0, inv_w = 1.0 / (c->p.damp_r1 - c->p.damp_r0);
-  const double tau0 = 2.0 * 3.14159265358979323846 * std::sqrt(r0 * r0 * r0 / c->p.gm_star);
   cudaStream_t s = c->stream;
   const double* Q0 = c->q0();
   const Geom g = c->g;
+  const DampArgs D = make_damp(c, dt);
   dispatch_m(c->L.m,
-             [&] { damp_kernel<1><<<grid, 128, 0, s>>>(Q, Q0, g, dt, r0, inv_w, tau0); },
-             [&] { damp_kernel<2><<<grid, 128, 0, s>>>(Q, Q0, g, dt, r0, inv_w, tau0); },
-             [&] { damp_kernel<3><<<grid, 128, 0, s>>>(Q, Q0, g, dt, r0, inv_w, tau0); },
-             [&] { damp_kernel<4><<<grid, 128, 0, s>>>(Q, Q0, g, dt, r0, inv_w, tau0); },
-             [&] { damp_kernel<5><<<grid, 128, 0, s>>>(Q, Q0, g, dt, r0, inv_w, tau0); });
+             [&] { damp_kernel<1><<<grid, 128, 0, s>>>(Q, Q0, g, D); },
+             [&] { damp_kernel<2><<<grid, 128, 0, s>>>(Q, Q0, g, D); },
+             [&] { damp_kernel<3><<<grid, 128, 0, s>>>(Q, Q0, g, D); },
+             [&] { damp_kernel<4><<<grid, 128, 0, s>>>(Q, Q0, g, D); },
+             [&] { damp_kernel<5><<<grid, 128, 0, s>>>(Q, Q0, g, D); });
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
   return DG_OK;
@@ -309,13 +329,7 @@ int launch_limit(dg_ctx* c, double* Q, bool final_, double dt) {
   LimitArgs A{};
   A.q = Q; A.q0 = c->q0(); A.wmax = c->wmax();
   A.eps = c->p.lim_eps > 0.0 ? c->p.lim_eps : 1e-13;
-  A.dt = dt;
-  const bool damp = final_ && c->p.damp_r0 > 0.0;
-  A.damp_r0 = damp ? c->p.damp_r0 : 0.0;
-  A.damp_inv_w = damp ? 1.0 / (c->p.damp_r1 - c->p.damp_r0) : 0.0;
-  A.damp_tau0 = damp ? 2.0 * 3.14159265358979323846 *
-                           std::sqrt(c->p.damp_r0 * c->p.damp_r0 * c->p.damp_r0 / c->p.gm_star)
-                     : 0.0;
+  A.D = make_damp(c, dt, final_);
   A.rows = c->rows_per_cta;
   A.g = c->g;
   A.ph = make_phys(c, c->t);
@@ -350,7 +364,7 @@ int do_step(dg_ctx* c, double dt, double* stages) {
   if (!(dt >= 0.0) || !std::isfinite(dt)) return fail(c, DG_EINVAL, "dg_step: bad dt");
   const int A = c->cur, B = (c->cur + 1) % 3, Cc = (c->cur + 2) % 3;
   const size_t n = (size_t)c->p.ny * c->p.nx * 4 * c->L.m * c->L.m;
-  const bool damp = c->p.damp_r0 > 0.0;
+  const bool damp = has_damping(c->p);
   const bool lim = c->p.limiter != 0;
   const bool fuse_tail = !stages && (c->fused_cfl || damp);   // damping + CFL ride on the step's last kernel
   int e;

@@ -61,6 +61,36 @@ struct Geom {
   int nx, ny, nbx, bc;
 };
 
+// Wave-killing zones (row a12): outer zone r > r0 (full strength from r1 outwards) and,
+// for the paper's own disc, an inner zone r < in_r0 (full strength from in_r1 inwards).  Per cell, with
+// the ramp R = min(1, ((r - r_d)/(r_b - r_d))^2) and tau = 2 pi sqrt(r_d^3/GM)/R:  Q <- f0 Q0 + ft Q,
+// f0 = dt/(tau + dt), ft = tau/(tau + dt).
+struct DampArgs {
+  double r0, inv_w, tau0;          // outer: r_d, 1/(r_b - r_d), 2 pi sqrt(r_d^3/GM); off: r0 = +inf, on = 0
+  double in_r0, in_inv_w, in_tau0; // inner: r_d, 1/(r_d - r_b), 2 pi sqrt(r_d^3/GM); off: in_r0 = 0
+  int on;                          // any zone enabled
+  double dt;
+};
+__device__ __forceinline__ bool damp_factors(const DampArgs& D, double rc, double& f0, double& ft) {
+  double s, tau0;
+  if (rc > D.r0) {                               // r0 = +inf when the outer zone is off
+    s = (rc - D.r0) * D.inv_w;
+    tau0 = D.tau0;
+  } else if (rc < D.in_r0) {                     // in_r0 = 0 when the inner zone is off
+    s = (D.in_r0 - rc) * D.in_inv_w;
+    tau0 = D.in_tau0;
+  } else {
+    return false;
+  }
+  const double R = fmin(1.0, s * s);
+  if (!(R > 0.0)) return false;
+  const double tau = tau0 / R;
+  const double inv = 1.0 / (tau + D.dt);
+  f0 = D.dt * inv;
+  ft = tau * inv;
+  return true;
+}
+
 struct StageArgs {
   const double* qprev;        // u^(s-1)
   const double* qn;           // u^n
@@ -69,7 +99,7 @@ struct StageArgs {
   const double* btrW; const double* btrE; const double* btrS; const double* btrN;  // bc 2 traces
   unsigned long long* wmax;   // CFL wave-speed maximum (bit pattern of a non-negative double)
   double a, b, dt;            // out = a u^n + b u^(s-1) + beta N; beta = b dt is folded into T and ph
-  double damp_r0, damp_inv_w, damp_tau0;
+  DampArgs D;
   int rows;
   // K_GEN / K_GENL: earlier slopes K_j = dt N(y_j) with their Butcher coefficients, this sub-step's own
   // coefficient, and where to keep K_i (null: not needed again)
@@ -292,10 +322,16 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   // the last stage also reads the initial state where the wave-killing zone is active: pull that
   // tile into L2 ahead of its use (cheap test on the tile's farthest corner)
   auto prefetch_q0 = [&](int j) {                // thread 0 only
-    const double xa = fmax(fabs(g.x0 + ib * 32 * g.dx), fabs(g.x0 + (ib * 32 + 32) * g.dx));
-    const double ya = fmax(fabs(g.y0 + j * g.dy), fabs(g.y0 + (j + 1) * g.dy));
-    if (xa * xa + ya * ya > A.damp_r0 * A.damp_r0)
-      bulk_prefetch_l2(A.q0 + (size_t)j * row_stride + (size_t)ib * BS, TILE_BYTES);
+    const double xl = g.x0 + ib * 32 * g.dx, xr = g.x0 + (ib * 32 + 32) * g.dx;
+    const double yl = g.y0 + j * g.dy, yr = g.y0 + (j + 1) * g.dy;
+    const double xa = fmax(fabs(xl), fabs(xr)), ya = fmax(fabs(yl), fabs(yr));
+    bool want = xa * xa + ya * ya > A.D.r0 * A.D.r0;
+    if (A.D.in_r0 > 0.0 && !want) {              // inner zone: the tile's nearest point to the origin
+      const double xn = (xl <= 0.0 && xr >= 0.0) ? 0.0 : fmin(fabs(xl), fabs(xr));
+      const double yn = (yl <= 0.0 && yr >= 0.0) ? 0.0 : fmin(fabs(yl), fabs(yr));
+      want = xn * xn + yn * yn < A.D.in_r0 * A.D.in_r0;
+    }
+    if (want) bulk_prefetch_l2(A.q0 + (size_t)j * row_stride + (size_t)ib * BS, TILE_BYTES);
   };
 
   // Butcher sub-steps read u^n and the earlier slopes in the epilogue: pull the row's tiles into L2 ahead
@@ -525,20 +561,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       // wave-killing factors of this cell (row a12): out <- f0 u0 + ft out
       double f0 = 0.0, ft = 1.0;
       bool damp = false;
-      if (do_damp && (KIND != K_GENL || A.damp_r0 > 0.0)) {
-        const double rc = sqrt(xc * xc + yc * yc);
-        if (rc > A.damp_r0) {
-          const double s = (rc - A.damp_r0) * A.damp_inv_w;
-          const double R = fmin(1.0, s * s);
-          if (R > 0.0) {
-            const double tau = A.damp_tau0 / R;
-            const double inv = 1.0 / (tau + A.dt);
-            damp = true;
-            f0 = A.dt * inv;
-            ft = tau * inv;
-          }
-        }
-      }
+      if (do_damp && (KIND != K_GENL || A.D.on))
+        damp = damp_factors(A.D, sqrt(xc * xc + yc * yc), f0, ft);
       // the initial state of the damped cells: for M <= 4 requested here and used in the epilogue (the
       // loads have the whole Y phase to land); at M = 5 the 20 extra live doubles cost more than they
       // save (measured: 0.668 vs 0.637 ms for the last stage), so there the loads stay in the epilogue
@@ -868,8 +892,7 @@ __global__ void boundary_trace_kernel(const double* __restrict__ Q0, double* btr
 // stage (dg_step_debug).  In place: Q <- (dt Q0 + tau Q)/(tau + dt) for cells with R(r) > 0.
 template <int M>
 __global__ void __launch_bounds__(128)
-damp_kernel(double* __restrict__ Q, const double* __restrict__ Q0, Geom g, double dt, double r0,
-            double inv_w, double tau0) {
+damp_kernel(double* __restrict__ Q, const double* __restrict__ Q0, Geom g, DampArgs D) {
   const int lane = threadIdx.x & 31;
   const int j = blockIdx.y * 4 + (threadIdx.x >> 5);
   const int ib = blockIdx.x;
@@ -877,15 +900,11 @@ damp_kernel(double* __restrict__ Q, const double* __restrict__ Q0, Geom g, doubl
   constexpr int C = 4 * M * M;
   if (j >= g.ny || i >= g.nx) return;
   const double xc = g.x0 + (i + 0.5) * g.dx, yc = g.y0 + (j + 0.5) * g.dy;
-  const double rc = sqrt(xc * xc + yc * yc);
-  if (!(rc > r0)) return;
-  const double s = (rc - r0) * inv_w;
-  const double R = fmin(1.0, s * s);
-  if (!(R > 0.0)) return;
-  const double tau = tau0 / R;
+  double f0, ft;
+  if (!damp_factors(D, sqrt(xc * xc + yc * yc), f0, ft)) return;
   const size_t base = ((size_t)j * g.nbx + ib) * C * 32 + lane;
 #pragma unroll 4
-  for (int e = 0; e < C; ++e) Q[base + e * 32] = (dt * Q0[base + e * 32] + tau * Q[base + e * 32]) / (tau + dt);
+  for (int e = 0; e < C; ++e) Q[base + e * 32] = fma(f0, Q0[base + e * 32], ft * Q[base + e * 32]);
 }
 
 }  // namespace dg

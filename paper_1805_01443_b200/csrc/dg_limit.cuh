@@ -30,7 +30,7 @@ struct LimitArgs {
   const double* q0;              // initial state (FINAL with damping)
   unsigned long long* wmax;      // FINAL: CFL wave-speed maximum
   double eps;                    // floor for density and pressure
-  double dt, damp_r0, damp_inv_w, damp_tau0;
+  DampArgs D;                    // FINAL: wave-killing zones (all off: no relaxation)
   int rows;
   Geom g;
   Phys ph;
@@ -77,7 +77,7 @@ limit_kernel(const __grid_constant__ LimitArgs A) {
   const int j0 = blockIdx.y * A.rows, j1 = min(g.ny, j0 + A.rows);
   const size_t row_stride = (size_t)g.nbx * BS;
   const double xc = g.x0 + (i + 0.5) * g.dx;
-  const bool damp_on = FINAL && A.damp_r0 > 0.0;
+  const bool damp_on = FINAL && A.D.on;
   double spmax = 0.0;
 
   auto cfl_of_row = [&](int j) {                 // warp 0: wave speed of row j from sAvg (row a10)
@@ -212,18 +212,7 @@ limit_kernel(const __grid_constant__ LimitArgs A) {
     bool damp = false;
     if (damp_on) {
       const double yc = g.y0 + (j + 0.5) * g.dy;
-      const double rc = sqrt(xc * xc + yc * yc);
-      if (rc > A.damp_r0) {
-        const double s = (rc - A.damp_r0) * A.damp_inv_w;
-        const double R = fmin(1.0, s * s);
-        if (R > 0.0) {
-          const double tau = A.damp_tau0 / R;
-          const double inv = 1.0 / (tau + A.dt);
-          damp = true;
-          f0 = A.dt * inv;
-          ft = tau * inv;
-        }
-      }
+      damp = damp_factors(A.D, sqrt(xc * xc + yc * yc), f0, ft);
     }
     const double* p0 = A.q0 + (size_t)j * row_stride + (size_t)ib * BS + lane;
     // (every thread read sAvg before the barrier that follows the sMin exchange: it may be rewritten now)

@@ -36,6 +36,7 @@ _PARAM_DEFAULTS = dict(
     q_planet=0.0, r_planet=1.0, eps_planet=0.0, omega_planet=1.0, phase0=0.0,
     damp_r0=0.0, damp_r1=0.0, t0=0.0,
     limiter=0, lim_eps=1e-13,
+    damp_in_r0=0.0, damp_in_r1=0.0,
 )
 
 
@@ -234,6 +235,36 @@ def disc(n: int = 256, order: int = 3, planet: bool = False, noise: float = 0.0,
         u = np.random.default_rng(NOISE_SEED).random((ny, nx, order, order))
         sigma = sigma * (1.0 + noise * (2.0 * u - 1.0))
     return p, project_nodal(p, _conservative(sigma, -om * Y, om * X, cs2 * sigma, gamma))
+
+
+def paper_disc(n: int = 256, order: int = 3, rk: int = 2, planet: bool = True, limiter: bool = True,
+               eps_star: float = 0.2, half_width: float = 2.25):
+    """The paper's own planet-disc setup: adiabatic disc
+    (gamma = 1.4), box [-2.25, 2.25]^2, Sigma = Sigma0/(1+f), p = p0/(1+f), f = exp((r - r_ex)/(r_p h)),
+    Sigma0 = 1, p0 = 2.5e-3, r_in = 0.4, r_ex = 1.75, h = 0.05; planet q = 6e-5 at r_p = 1, eps_p = 0.03;
+    v_phi^2 = r^2 Omega^2 - r c_iso^2 f / (r_p h (1+f)) with c_iso^2 = p0/Sigma0 (reading G12) and
+    Omega^2 = GM/r_in^3 inside r_in, GM/r^3 outside (reading G11: solid rotation inside, PAPER.md:288);
+    wave-killing zones r_d = r_in 1.15^(3/2) -> r_in and r_d = r_ex 1.15^(-3/2) -> r_ex; frozen box edge
+    (G14).  The density falls to ~4e-13 in the box corners: the positivity limiter is on by default.
+    The paper does not soften the star's potential; with eps_star = 0 the four cells around the origin blow up within
+    one step on a Cartesian grid, so the default is the BASELINE disc's 0.2 (inside the damped hole r < r_in)."""
+    h, gm, gamma = 0.05, 1.0, 1.4
+    r_in, r_ex, sigma0, p0 = 0.4, 1.75, 1.0, 2.5e-3
+    p = make_params(nx=n, ny=n, x0=-half_width, x1=half_width, y0=-half_width, y1=half_width,
+                    order=order, rk=rk, bc=2, eos=0, gamma=gamma, h_aspect=h, gm_star=gm, eps_star=eps_star,
+                    q_planet=6.0e-5 if planet else 0.0, r_planet=1.0, eps_planet=0.03, omega_planet=1.0,
+                    phase0=0.0, damp_r0=r_ex * 1.15 ** -1.5, damp_r1=r_ex,
+                    damp_in_r0=r_in * 1.15 ** 1.5, damp_in_r1=r_in,
+                    limiter=1 if limiter else 0, lim_eps=1e-13)
+    X, Y = _mesh(p)
+    r = np.sqrt(X * X + Y * Y)
+    f = np.exp((r - r_ex) / h)
+    sigma = sigma0 / (1.0 + f)
+    pr = p0 / (1.0 + f)
+    om2 = np.where(r <= r_in, gm / r_in ** 3, gm / np.maximum(r, 1e-300) ** 3)
+    vphi2 = r * r * om2 - r * (p0 / sigma0) * f / (h * (1.0 + f))
+    om = np.sqrt(np.maximum(vphi2, 0.0)) / np.maximum(r, 1e-300)
+    return p, project_nodal(p, _conservative(sigma, -om * Y, om * X, pr, gamma))
 
 
 LITERAL_BASELINE_DISC = dict(floor=1e-6, taper=0.05, eps_star=0.02)   # BASELINE.json's numbers (need a limiter)

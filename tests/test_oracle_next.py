@@ -352,3 +352,59 @@ def test_gresho_dg2_density_error_soft_pin():
     err = W.l1_error_percent(p, r.get_state(), np.ones_like(X))
     ref = _gresho_table()["DG2"][1]
     assert ref / 3 < err < ref * 3, err
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-3: the paper's own disc and its two wave-killing zones
+def test_inner_and_outer_damping_zones_hand_values():
+    """tau = 2 pi sqrt(r_d^3/GM)/R, R = ((r - r_d)/(r_b - r_d))^2 (clamped to 1 beyond r_b),
+    Q <- (dt Q0 + tau Q)/(tau + dt), i.e. Q0 + tau/(tau+dt) (Q - Q0); cells between the zones are untouched.
+    ref_step_debug returns the last sub-step's result before damping, the state afterwards is damped."""
+    n, m = 40, 2
+    p, U0 = W.random_smooth(n, n, m, seed=11, eos=0, bc=2, rk=2, gravity=True)
+    p.update(damp_r0=0.9, damp_r1=1.2, damp_in_r0=0.4, damp_in_r1=0.3)
+    r = oracle.RefDG(p)
+    r.set_state(U0)
+    dt = r.cfl_dt(0.2)
+    stages = r.step_debug(dt)
+    after = r.get_state()
+    assert np.isfinite(after).all()
+    xc = p["x0"] + (np.arange(n) + 0.5) * (p["x1"] - p["x0"]) / n
+    yc = p["y0"] + (np.arange(n) + 0.5) * (p["y1"] - p["y0"]) / n
+    rr = np.hypot(xc[None, :], yc[:, None])
+    out, inn = rr > 0.9, rr < 0.4
+    ft = np.ones((n, n))
+    R = np.minimum(1.0, ((rr - 0.9) / 0.3) ** 2)
+    tau = 2 * math.pi * math.sqrt(0.9 ** 3) / np.where(out, R, 1.0)
+    ft = np.where(out, tau / (tau + dt), ft)
+    R = np.minimum(1.0, ((0.4 - rr) / 0.1) ** 2)
+    tau = 2 * math.pi * math.sqrt(0.4 ** 3) / np.where(inn, R, 1.0)
+    ft = np.where(inn, tau / (tau + dt), ft)
+    assert inn.sum() > 4 and out.sum() > 100 and (~inn & ~out).sum() > 100
+    pred = U0 + ft[:, :, None, None, None] * (stages[-1] - U0)
+    np.testing.assert_allclose(after, pred, rtol=1e-13, atol=1e-13)
+    mid = ~inn & ~out
+    np.testing.assert_array_equal(after[mid], stages[-1][mid])
+    assert np.abs(after - stages[-1])[inn].max() > 1e-9 and np.abs(after - stages[-1])[out].max() > 1e-9
+
+
+def test_paper_disc_needs_and_survives_with_the_limiter():
+    """density ~4e-13 in the box corners.  With the limiter the run stays finite and
+    admissible at the cell averages; the initial data are the paper's (uniform Sigma0, p0 inside r_ex)."""
+    p, U = W.paper_disc(32, 3)
+    nod = W.evaluate_nodal(p, U)
+    X, Y = W._mesh(p)
+    rr = np.hypot(X, Y)
+    ring = (rr > 0.6) & (rr < 1.4)
+    np.testing.assert_allclose(nod[:, :, 0][ring], 1.0, rtol=2e-3)
+    pr = 0.4 * (nod[:, :, 3] - 0.5 * (nod[:, :, 1] ** 2 + nod[:, :, 2] ** 2) / nod[:, :, 0])
+    np.testing.assert_allclose(pr[ring], 2.5e-3, rtol=5e-2)
+    assert nod[:, :, 0].min() < 1e-11
+    assert abs(p["damp_in_r0"] - 0.4 * 1.15 ** 1.5) < 1e-15 and abs(p["damp_r0"] - 1.75 * 1.15 ** -1.5) < 1e-15
+    r = oracle.RefDG(p, omp=True)
+    r.set_state(U)
+    r.limit()
+    for _ in range(60):
+        r.step(r.cfl_dt(0.2))
+    S = r.get_state()
+    assert np.isfinite(S).all() and S[..., 0, 0, 0].min() > 0

@@ -414,3 +414,51 @@ def test_gresho_table1_soft_pin_on_gpu(DG):
     assert errs[2] > errs[3] > errs[4], errs
     for m in (2, 3, 4):
         assert table[m] / 4 < errs[m] < table[m] * 4, errs
+
+
+@pytest.mark.parametrize("m,rk", [(3, 2), (5, 5)])
+def test_paper_disc_100_steps(DG, m, rk):
+    """The paper's own disc (NEXT-3): adiabatic, limiter on (density 4e-13 in the box
+    corners), inner and outer wave-killing zones, planet q = 6e-5; 100 free-running steps within 1e-10 and
+    the torque of Eq.(6) on the final state."""
+    n = 48 if m == 3 else 32
+    p, U = W.paper_disc(n, m, rk=rk)
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    ref.limit()
+    U1 = ref.get_state()
+    ref.set_state(U1)
+    g = DG(p)
+    g.set_state(dev(U))
+    g.limit()                                              # dg_limit on the freshly projected state
+    assert rel_err(g.get_state().cpu().numpy(), U1) < TOL_STAGE
+    g.set_state(dev(U1))
+    for _ in range(100):
+        dt_ref = ref.cfl_dt(0.2)
+        assert abs(g.cfl_dt(0.2) / dt_ref - 1.0) < 1e-9
+        ref.step(dt_ref)
+        g.step(dt_ref)
+    out = g.get_state().cpu().numpy()
+    assert np.isfinite(out).all()
+    assert rel_err(out, ref.get_state()) < TOL_100
+    t = ref.time
+    gr = ref.torque(t)
+    assert abs(g.torque(t) - gr) < 1e-9 * max(1.0, abs(gr))
+
+
+def test_inner_damping_zone_stage_parity(DG):
+    p, U = W.random_smooth(70, 33, 4, seed=12, eos=0, bc=2, rk=3, gravity=True)
+    p.update(damp_r0=0.9, damp_r1=1.2, damp_in_r0=0.4, damp_in_r1=0.3)
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    dt = ref.cfl_dt(0.2)
+    ref.step(dt)
+    for lim in (0, 1):
+        g = DG(dict(p, limiter=lim))
+        g.set_state(dev(U))
+        g.step(dt)                                         # fused tail: stage kernel (lim 0) / limiter pass (lim 1)
+        assert rel_err(g.get_state().cpu().numpy(), ref.get_state()) < TOL_STAGE
+        g2 = DG(dict(p, limiter=lim))
+        g2.set_state(dev(U))
+        g2.step_debug(dt)                                  # stand-alone damping kernel
+        assert rel_err(g2.get_state().cpu().numpy(), ref.get_state()) < TOL_STAGE
