@@ -143,6 +143,7 @@ long long dg_launch_count(const dg_ctx*);
  *   DG_TUNE_FUSED_CFL    : 1 = the last RK stage also reduces the CFL wave speed (default), 0 = separate kernel */
 #define DG_TUNE_ROWS_PER_CTA 1
 #define DG_TUNE_FUSED_CFL    2
+#define DG_TUNE_GEN_PREFETCH 3   /* Butcher sub-steps: L2 prefetch of u^n / earlier slopes: 0 none, 1 at the start of the row, 2 a row ahead, 3 between the x and y phases of the row (default) */
 int dg_set_tuning(dg_ctx*, int key, int value);
 
 /* Average-duration probe: enqueue CUDA events around the stage kernels of the next dg_step calls.

@@ -95,6 +95,7 @@ struct dg_ctx {
   double t;
   int rows_per_cta;
   int fused_cfl;
+  int gen_pf;
   long long launches;
   bool timing;
   std::vector<cudaEvent_t> evs;      // pairs (start, stop) around stage kernels, recorded without syncing
@@ -196,7 +197,7 @@ int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout,
   const bool gen = kind == K_GEN || kind == K_GENL;
   const double beta = kind == K_RHS ? 1.0 : (gen ? dt : b * dt);
   if (gen) {
-    A.nk = ga->nk; A.kself = ga->kself; A.kout = ga->kout;
+    A.nk = ga->nk; A.kself = ga->kself; A.kout = ga->kout; A.gen_pf = c->gen_pf;
     for (int k = 0; k < ga->nk; ++k) { A.kin[k] = ga->kin[k]; A.kc[k] = ga->kc[k]; }
   }
   A.qprev = qprev; A.qn = qn; A.qout = qout; A.q0 = c->q0();
@@ -451,6 +452,7 @@ int dg_init(const dg_params* p, void* workspace, size_t ws_bytes, void* cuda_str
   c->t = p->t0;
   c->rows_per_cta = 16;
   c->fused_cfl = 1;
+  c->gen_pf = 3;
   c->launches = 0;
   c->timing = false;
   c->ev_used = 0;
@@ -630,6 +632,10 @@ int dg_set_tuning(dg_ctx* c, int key, int value) {
     case DG_TUNE_FUSED_CFL:
       c->fused_cfl = value ? 1 : 0;
       c->wmax_valid = false;
+      return DG_OK;
+    case DG_TUNE_GEN_PREFETCH:
+      if (value < 0 || value > 3) return fail(c, DG_EINVAL, "prefetch mode must be 0..3");
+      c->gen_pf = value;
       return DG_OK;
     default:
       return fail(c, DG_EINVAL, "unknown tuning key");

@@ -108,6 +108,7 @@ struct StageArgs {
   double kself;
   double* kout;
   int nk;
+  int gen_pf;                 // L2 prefetch of the epilogue's inputs: 0 none, 1 row start, 2 a row ahead (evicted before use: 1.7x DRAM reads), 3 at the x/y phase boundary
   Geom g;
   Phys ph;
   DevTables T;
@@ -353,7 +354,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     tile_issue(2);
     if (use_un) un_issue(j0);
     if (do_damp) prefetch_q0(j0);
-    if (gen) prefetch_gen(j0);
+    if (gen && A.gen_pf) prefetch_gen(j0);
   }
 
   // line r = w of the two out-of-block x-neighbours, fetched one row ahead (lanes 0..7)
@@ -401,7 +402,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       if (more) tile_issue(t + 2);               // row j+2 -> the slot row j-1 has just left
       if (use_un && j > j0) un_issue(j);         // sN is free again
       if (do_damp && more) prefetch_q0(j + 1);
-      if (gen && more) prefetch_gen(j + 1);
+      if (gen && A.gen_pf == 2 && more) prefetch_gen(j + 1);
+      if (gen && A.gen_pf == 1 && j > j0) prefetch_gen(j);
     }
     const double* tu = tiles + (t % NST) * BS + lane;
     const double yc = g.y0 + (j + 0.5) * g.dy;
@@ -549,6 +551,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     }
     __syncthreads();
 
+    if (gen && A.gen_pf == 3 && tid == 32 % (M * 32)) prefetch_gen(j);
     // =========================== Y phase: xi-column q = w ===========================
     {
       const int q = w;
