@@ -3,7 +3,7 @@
  * Plain, slow, single-threaded (optionally one `omp parallel for` over cell rows) fp64 restatement
  * of the explicit modal DG right-hand side + SSP-RK stage update of arXiv:1805.01443 for the 2D
  * Euler equations, written step by step in the paper's order and notation (SURVEY.md section 8(c),
- * items C1..C11).  Host pointers only.  Shares no code, header, table or constant generator with
+ * items C1..C11; C8b, C12, C13 for the rows of SURVEY.md 8(f)).  Host pointers only.  Shares no code, header, table or constant generator with
  * the CUDA path (paper_1805_01443_b200/csrc, include/dg.h); neither includes the other.
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * load this library.
