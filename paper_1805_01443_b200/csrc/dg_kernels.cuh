@@ -421,11 +421,11 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       double sp = 0.0;
       if (valid) {
         const double ycp = g.y0 + (j - 0.5) * g.dy;
-        const double rinv = 1.0 / avg[0];
+        const double rinv = rcp_fast(avg[0]);    // slow-path-free: this warp is the row's critical path
         const double vx = avg[1] * rinv, vy = avg[2] * rinv;
         double c;
-        if (EOS == 0) c = sqrt(A.ph.gamma * A.ph.gm1 * (avg[3] - 0.5 * (avg[1] * vx + avg[2] * vy)) * rinv);
-        else          c = sqrt(A.ph.h2gm * rsqrt(fma(xc, xc, fma(ycp, ycp, A.ph.eps2s))));
+        if (EOS == 0) c = sqrt_fast(A.ph.gamma * A.ph.gm1 * (avg[3] - 0.5 * (avg[1] * vx + avg[2] * vy)) * rinv);
+        else          c = sqrt_fast(A.ph.h2gm * rsqrt_fast(fma(xc, xc, fma(ycp, ycp, A.ph.eps2s))));
         sp = (fabs(vx) + c) * g.inv_dx + (fabs(vy) + c) * g.inv_dy;
         if (!(sp >= 0.0)) sp = __longlong_as_double(0x7ff0000000000000LL);   // NaN -> +inf
       }
