@@ -462,3 +462,23 @@ def test_inner_damping_zone_stage_parity(DG):
         g2.set_state(dev(U))
         g2.step_debug(dt)                                  # stand-alone damping kernel
         assert rel_err(g2.get_state().cpu().numpy(), ref.get_state()) < TOL_STAGE
+
+
+def test_full_size_next_rows(DG):
+    """BASELINE configs[3]'s grid (1024^2, order 5) with the 8(f) rows switched on: Cash-Karp + limiter, one
+    full step (6 sub-steps, 6 limiter passes, fused tail) against the OpenMP oracle on every element, then
+    the torque of the result."""
+    p, U = W.disc(1024, 5, planet=True, noise=1e-4, rk=5)
+    p = dict(p, limiter=1)
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    g = DG(p)
+    g.set_state(dev(U))
+    dt = ref.cfl_dt(0.2)
+    assert abs(g.cfl_dt(0.2) / dt - 1.0) < 1e-13
+    ref.step(dt)
+    g.step(dt)
+    assert rel_err(g.get_state().cpu().numpy(), ref.get_state()) < TOL_STAGE
+    assert abs(g.cfl_dt(0.2) / ref.cfl_dt(0.2) - 1.0) < 1e-12
+    gr = ref.torque(ref.time)
+    assert abs(g.torque(ref.time) - gr) < 1e-11 * max(1.0, abs(gr))
