@@ -446,8 +446,9 @@ def test_paper_disc_100_steps(DG, m, rk):
     assert abs(g.torque(t) - gr) < 1e-9 * max(1.0, abs(gr))
 
 
-def test_inner_damping_zone_stage_parity(DG):
-    p, U = W.random_smooth(70, 33, 4, seed=12, eos=0, bc=2, rk=3, gravity=True)
+@pytest.mark.parametrize("rk", [3, 4])
+def test_inner_damping_zone_stage_parity(DG, rk):
+    p, U = W.random_smooth(70, 33, 4, seed=12, eos=0, bc=2, rk=rk, gravity=True)
     p.update(damp_r0=0.9, damp_r1=1.2, damp_in_r0=0.4, damp_in_r1=0.3)
     ref = oracle.RefDG(p, omp=True)
     ref.set_state(U)
