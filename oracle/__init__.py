@@ -43,6 +43,7 @@ class RefParams(C.Structure):
         ("omega_planet", C.c_double), ("phase0", C.c_double),
         ("damp_r0", C.c_double), ("damp_r1", C.c_double), ("t0", C.c_double),
         ("limiter", C.c_int32), ("lim_eps", C.c_double),
+        ("flux", C.c_int32),
         ("damp_in_r0", C.c_double), ("damp_in_r1", C.c_double),
     ]
 
@@ -76,6 +77,7 @@ def _lib(omp: bool):
         "ref_tables": (i, [i, _PD, _PD, _PD, _PD, _PD, _PD]),
         "ref_point_flux": (i, [PP, _PD, d, d, i, _PD, _PD, _PD]),
         "ref_llf": (i, [PP, _PD, _PD, d, d, i, _PD]),
+        "ref_hllc": (i, [PP, _PD, _PD, d, d, i, _PD]),
         "ref_gravity": (i, [PP, d, d, d, _PD]),
         "ref_rhs_parts": (i, [vp, d, i, _PD]), "ref_damp": (i, [vp, d]),
         "ref_rk_step": (i, [i, C.c_long, _PD, d, d, _ODE_FN, vp, _PD]),
@@ -223,6 +225,16 @@ def llf(params: dict, UL, UR, x: float, y: float, direction: int) -> np.ndarray:
     UR = np.ascontiguousarray(UR, dtype=np.float64)
     H = np.empty(4)
     _chk(L.ref_llf(C.byref(_to_struct(params)), _p(UL), _p(UR), x, y, direction, _p(H)), "ref_llf")
+    return H
+
+
+def hllc(params: dict, UL, UR, x: float, y: float, direction: int) -> np.ndarray:
+    """C5b: HLLC (eos 0) / HLL (eos 1) flux across a face with normal +direction."""
+    L = _lib(False)
+    UL = np.ascontiguousarray(UL, dtype=np.float64)
+    UR = np.ascontiguousarray(UR, dtype=np.float64)
+    H = np.empty(4)
+    _chk(L.ref_hllc(C.byref(_to_struct(params)), _p(UL), _p(UR), x, y, direction, _p(H)), "ref_hllc")
     return H
 
 

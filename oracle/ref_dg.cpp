@@ -6,6 +6,7 @@
  *   C3  Euler fluxes    PAPER.md:36-43  Eq.(1)
  *   C4  EOS             PAPER.md:45-49  Eq.(2); locally isothermal closure from BASELINE.json
  *   C5  numerical flux  PAPER.md:97  (type unnamed; BASELINE cfg0: local Lax-Friedrichs)
+ *   C5b HLLC / HLL flux option (PAPER.md:97 leaves the flux unnamed)
  *   C6  gravity source
  *   C7  RHS             PAPER.md:85-97  Eq.(3), divided by the (diagonal) mass
  *   C8  SSP-RK          PAPER.md:105-111 (Gottlieb & Shu 1998, Shu-Osher form)
@@ -145,6 +146,47 @@ void llf(const ref_params& p, const double* UL, const double* UR, double x, doub
   for (int v = 0; v < NV; ++v) H[v] = 0.5 * (FL[v] + FR[v]) - 0.5 * lam * (UR[v] - UL[v]);
 }
 
+/* C5b: HLL-type fluxes with the wave-speed estimates of Davis (1988),
+ *   S_L = min(v_L - c_L, v_R - c_R),  S_R = max(v_L + c_L, v_R + c_R).
+ * eos 1 (isothermal, no contact wave):  HLL  H = (S_R F_L - S_L F_R + S_L S_R (U_R - U_L))/(S_R - S_L) for
+ * S_L < 0 < S_R, else the upwind flux.  eos 0: HLLC (Toro, Spruce & Speares 1994) with the contact speed
+ *   S* = (p_R - p_L + rho_L v_L (S_L - v_L) - rho_R v_R (S_R - v_R)) / (rho_L (S_L - v_L) - rho_R (S_R - v_R))
+ * and the star states U*_K = rho_K (S_K - v_K)/(S_K - S*) (1, S* | v_t, E_K/rho_K + (S* - v_K)(S* + p_K/(rho_K (S_K - v_K)))),
+ * H = F_L | F_L + S_L (U*_L - U_L) | F_R + S_R (U*_R - U_R) | F_R  for  0 <= S_L | S_L <= 0 <= S* | S* <= 0 <= S_R | S_R <= 0. */
+void hllc(const ref_params& p, const double* UL, const double* UR, double x, double y, int dir, double* H) {
+  double FL[NV], FR[NV], vL, vR, cL, cR;
+  point_flux(p, UL, x, y, dir, FL, &vL, &cL);
+  point_flux(p, UR, x, y, dir, FR, &vR, &cR);
+  const double SL = std::fmin(vL - cL, vR - cR), SR = std::fmax(vL + cL, vR + cR);
+  if (SL >= 0.0) { for (int v = 0; v < NV; ++v) H[v] = FL[v]; return; }
+  if (SR <= 0.0) { for (int v = 0; v < NV; ++v) H[v] = FR[v]; return; }
+  if (p.eos == 1) {
+    for (int v = 0; v < NV; ++v) H[v] = (SR * FL[v] - SL * FR[v] + SL * SR * (UR[v] - UL[v])) / (SR - SL);
+    return;
+  }
+  const int n = 1 + dir, tg = 2 - dir;               /* normal and tangential momentum components */
+  const double pL = (p.gamma - 1.0) * (UL[3] - 0.5 * (UL[1] * UL[1] + UL[2] * UL[2]) / UL[0]);
+  const double pR = (p.gamma - 1.0) * (UR[3] - 0.5 * (UR[1] * UR[1] + UR[2] * UR[2]) / UR[0]);
+  const double mL = UL[0] * (SL - vL), mR = UR[0] * (SR - vR);
+  const double Ss = (pR - pL + UL[n] * (SL - vL) - UR[n] * (SR - vR)) / (mL - mR);
+  const double* U = Ss >= 0.0 ? UL : UR;
+  const double* F = Ss >= 0.0 ? FL : FR;
+  const double S = Ss >= 0.0 ? SL : SR, vK = Ss >= 0.0 ? vL : vR, pK = Ss >= 0.0 ? pL : pR;
+  const double fac = U[0] * (S - vK) / (S - Ss);
+  double Us[NV];
+  Us[0] = fac;
+  Us[n] = fac * Ss;
+  Us[tg] = fac * (U[tg] / U[0]);
+  Us[3] = fac * (U[3] / U[0] + (Ss - vK) * (Ss + pK / (U[0] * (S - vK))));
+  for (int v = 0; v < NV; ++v) H[v] = F[v] + S * (Us[v] - U[v]);
+}
+
+/* the numerical flux selected by params.flux */
+inline void num_flux(const ref_params& p, const double* UL, const double* UR, double x, double y, int dir, double* H) {
+  if (p.flux == 1) hllc(p, UL, UR, x, y, dir, H);
+  else llf(p, UL, UR, x, y, dir, H);
+}
+
 /* C6 */
 void gravity(const ref_params& p, double t, double x, double y, double* g) {
   g[0] = 0.0; g[1] = 0.0;
@@ -247,7 +289,7 @@ void compute_rhs(const ref_ctx* c, const double* U, double t, int parts, double*
             if (p.bc == 1) std::memcpy(UR, UL, sizeof UR);
             else trace_x(c, c->U0.data(), nx - 1, j, +1, r, UR);
           }
-          llf(p, UL, UR, xf, yr, 0, &HX[(((size_t)j * (nx + 1) + f) * m + r) * NV]);
+          num_flux(p, UL, UR, xf, yr, 0, &HX[(((size_t)j * (nx + 1) + f) * m + r) * NV]);
         }
 #pragma omp parallel for schedule(static)
     for (int f = 0; f <= ny; ++f)
@@ -271,7 +313,7 @@ void compute_rhs(const ref_ctx* c, const double* U, double t, int parts, double*
             if (p.bc == 1) std::memcpy(UR, UL, sizeof UR);
             else trace_y(c, c->U0.data(), i, ny - 1, +1, q, UR);
           }
-          llf(p, UL, UR, xq, yf, 1, &HY[(((size_t)f * nx + i) * m + q) * NV]);
+          num_flux(p, UL, UR, xq, yf, 1, &HY[(((size_t)f * nx + i) * m + q) * NV]);
         }
   }
 
@@ -567,6 +609,7 @@ int check_params(const ref_params* p) {
   if (p->eos == 1 && !(p->h_aspect > 0.0 && p->gm_star > 0.0)) return -1;
   if (p->damp_r0 > 0.0 && !(p->damp_r1 > p->damp_r0 && p->gm_star > 0.0)) return -1;
   if (p->limiter != 0 && p->limiter != 1) return -1;
+  if (p->flux != 0 && p->flux != 1) return -1;
   if (p->limiter == 1 && !(p->lim_eps > 0.0)) return -1;
   if (p->damp_in_r0 > 0.0 && !(p->damp_in_r1 >= 0.0 && p->damp_in_r1 < p->damp_in_r0 && p->gm_star > 0.0)) return -1;
   return 0;
@@ -777,6 +820,13 @@ int ref_llf(const ref_params* p, const double* UL, const double* UR, double x, d
             double* H4) {
   if (!p || (dir != 0 && dir != 1)) return -1;
   llf(*p, UL, UR, x, y, dir, H4);
+  return 0;
+}
+
+int ref_hllc(const ref_params* p, const double* UL, const double* UR, double x, double y, int dir,
+             double* H4) {
+  if (!p || (dir != 0 && dir != 1)) return -1;
+  hllc(*p, UL, UR, x, y, dir, H4);
   return 0;
 }
 

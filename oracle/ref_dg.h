@@ -38,6 +38,8 @@ typedef struct {
   int32_t limiter;           /* 1: positivity-preserving limiter (Zhang & Shu 2010) after every
                                 RK sub-step and the w_1/2 factor in the time step */
   double  lim_eps;           /* the limiter's floor for density and pressure (Zhang & Shu use 1e-13) */
+  int32_t flux;              /* numerical flux h_{e,K} (type unnamed): 0 local Lax-Friedrichs (C5);
+                                1 HLLC (eos 0; Toro, Spruce & Speares 1994) / HLL (eos 1), Davis wave speeds (C5b) */
   double  damp_in_r0, damp_in_r1; /* inner wave-killing zone r < damp_in_r0 (r_d = r_in 1.15^(3/2),
                                      boundary radius r_in = damp_in_r1); damp_in_r0 <= 0: off */
 } ref_params;
@@ -66,6 +68,9 @@ int  ref_point_flux(const ref_params*, const double* U4, double x, double y, int
 /* C5: local Lax-Friedrichs flux across a face with normal +dir, left state UL, right state UR. */
 int  ref_llf(const ref_params*, const double* UL, const double* UR, double x, double y, int dir,
              double* H4);
+/* C5b: HLLC (eos 0) / HLL (eos 1) flux, same arguments as ref_llf. */
+int  ref_hllc(const ref_params*, const double* UL, const double* UR, double x, double y, int dir,
+              double* H4);
 /* C6: gravitational acceleration g = -grad Phi at (x,y), time t. */
 int  ref_gravity(const ref_params*, double t, double x, double y, double* g2);
 /* C7 split: parts bitmask 1 = volume flux term, 2 = face term, 4 = source term. */

@@ -35,7 +35,7 @@ _PARAM_DEFAULTS = dict(
     gm_star=0.0, eps_star=0.0,
     q_planet=0.0, r_planet=1.0, eps_planet=0.0, omega_planet=1.0, phase0=0.0,
     damp_r0=0.0, damp_r1=0.0, t0=0.0,
-    limiter=0, lim_eps=1e-13,
+    limiter=0, lim_eps=1e-13, flux=0,
     damp_in_r0=0.0, damp_in_r1=0.0,
 )
 

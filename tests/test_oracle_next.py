@@ -408,3 +408,98 @@ def test_paper_disc_needs_and_survives_with_the_limiter():
         r.step(r.cfl_dt(0.2))
     S = r.get_state()
     assert np.isfinite(S).all() and S[..., 0, 0, 0].min() > 0
+
+
+# ------------------------------------------------------------------------------------------------
+# C5b: HLLC / HLL flux option
+def _flux_of(p, U, d):
+    return oracle.point_flux(p, U, 0.3, -0.2, d)[0]
+
+
+@pytest.mark.parametrize("eos", [0, 1])
+@pytest.mark.parametrize("direction", [0, 1])
+def test_hllc_consistency_upwinding_and_mirror_symmetry(eos, direction):
+    kw = dict(eos=1, h_aspect=0.3, gm_star=1.0, eps_star=0.1) if eos else dict(eos=0)
+    p = W.make_params(nx=1, ny=1, order=1, gamma=1.4, flux=1, **kw)
+    rng = np.random.default_rng(3 + direction)
+    nrm = 1 + direction
+    for _ in range(40):
+        UL = np.array([1.0, 0.3, -0.2, 2.5]) + 0.1 * rng.normal(size=4)
+        UR = np.array([1.1, -0.4, 0.1, 2.2]) + 0.1 * rng.normal(size=4)
+        # consistency h(U,U) = f(U).n
+        np.testing.assert_allclose(oracle.hllc(p, UL, UL, 0.3, -0.2, direction), _flux_of(p, UL, direction),
+                                   rtol=1e-14, atol=1e-15)
+        # mirror: swap sides, flip the normal momentum -> the flux flips accordingly (single-valued, conservative)
+        H = oracle.hllc(p, UL, UR, 0.3, -0.2, direction)
+        ML, MR = UL.copy(), UR.copy()
+        ML[nrm] *= -1
+        MR[nrm] *= -1
+        sign = -np.ones(4)
+        sign[nrm] = 1.0
+        np.testing.assert_allclose(oracle.hllc(p, MR, ML, 0.3, -0.2, direction), sign * H, rtol=1e-13, atol=1e-14)
+        # supersonic to the right / left: pure upwinding
+        SL, SR = UL.copy(), UR.copy()
+        SL[nrm] = 9.0 * SL[0]
+        SR[nrm] = 8.0 * SR[0]
+        SL[3] += 0.5 * 81 * SL[0]
+        SR[3] += 0.5 * 64 * SR[0]
+        np.testing.assert_array_equal(oracle.hllc(p, SL, SR, 0.3, -0.2, direction), _flux_of(p, SL, direction))
+        SL[nrm] *= -1
+        SR[nrm] *= -1
+        np.testing.assert_array_equal(oracle.hllc(p, SL, SR, 0.3, -0.2, direction), _flux_of(p, SR, direction))
+
+
+@pytest.mark.parametrize("direction", [0, 1])
+def test_hllc_keeps_a_stationary_contact_exactly(direction):
+    """The defining property of HLLC (and what LLF lacks): across a contact at rest -- equal pressure, zero
+    normal velocity, any density and tangential-velocity jump -- the flux is (0, p n, 0): no mass, tangential
+    momentum or energy crosses.  The LLF flux of the same pair has a mass flux of lambda (rho_L - rho_R)/2."""
+    p = W.make_params(nx=1, ny=1, order=1, eos=0, gamma=1.4, flux=1)
+    pr = 0.7
+    nrm, tg = 1 + direction, 2 - direction
+    UL, UR = np.zeros(4), np.zeros(4)
+    UL[0], UR[0] = 2.0, 0.25
+    UL[tg], UR[tg] = 2.0 * 0.3, 0.25 * (-0.8)
+    UL[3] = pr / 0.4 + 0.5 * UL[tg] ** 2 / UL[0]
+    UR[3] = pr / 0.4 + 0.5 * UR[tg] ** 2 / UR[0]
+    H = oracle.hllc(p, UL, UR, 0.0, 0.0, direction)
+    ref = np.zeros(4)
+    ref[nrm] = pr
+    np.testing.assert_allclose(H, ref, rtol=0, atol=5e-16)
+    assert abs(oracle.llf(p, UL, UR, 0.0, 0.0, direction)[0]) > 0.5
+
+
+def test_hllc_dg_operator_is_conservative_and_preserves_free_stream():
+    p, U = W.random_smooth(9, 7, 3, seed=21, bc=0, rk=3)
+    p["flux"] = 1
+    r = oracle.RefDG(p)
+    r.set_state(U)
+    L = r.rhs(0.0)
+    dxdy = 1.0
+    tot = L[..., 0, 0].sum(axis=(0, 1))
+    scale = np.abs(L[..., 0, 0]).sum(axis=(0, 1))
+    assert (np.abs(tot) / scale).max() < 1e-13
+    U0 = np.zeros_like(U)
+    U0[..., 0, 0] = [1.3, 0.4, -0.7, 2.9]
+    r.set_state(U0)
+    assert np.abs(r.rhs(0.0)).max() < 1e-11
+    # and it is a different operator from the LLF one on rough data
+    r2 = oracle.RefDG(dict(p, flux=0))
+    r2.set_state(U)
+    r.set_state(U)
+    assert np.abs(r.rhs(0.0) - r2.rhs(0.0)).max() > 1e-4
+
+
+def test_hllc_vortex_converges_at_design_order():
+    errs = []
+    for n in (8, 16):
+        p, U = W.vortex(n, 3, rk=3)
+        p["flux"] = 1
+        r = oracle.RefDG(p, omp=True)
+        r.set_state(U)
+        while r.time < 1.0:
+            r.step(min(r.cfl_dt(0.2), 1.0 - r.time))
+        X, Y = W._mesh(p)
+        exact = W.vortex_exact(X, Y, r.time)[0]
+        errs.append(np.abs(W.evaluate_nodal(p, r.get_state())[:, :, 0] - exact).mean())
+    assert math.log2(errs[0] / errs[1]) > 2.4, errs
