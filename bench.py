@@ -460,7 +460,7 @@ def run_variants(args):
     n, m = args.n, args.order
     for name, over in (("ssp33 (bench)", {}), ("ssp33 + limiter", {"limiter": 1}),
                        ("rk4: SSP-RK(5,4), paper Table 1", {"rk": 4}), ("rk5: Cash-Karp, paper Table 2", {"rk": 5}),
-                       ("rk5 + limiter", {"rk": 5, "limiter": 1})):
+                       ("rk5 + limiter", {"rk": 5, "limiter": 1}), ("ssp33, HLL flux (isothermal)", {"flux": 1})):
         p, U = W.disc(n, m, planet=True, noise=1e-4)
         p.update(over)
         g = DG(p)
@@ -482,7 +482,7 @@ def run_variants(args):
         arrays = step_arrays(p, acct["damping_zone_fraction"])
         sub = {2: 2, 3: 3, 4: 5, 5: 6}[p["rk"]]
         gbs = arrays * acct["state_bytes"] / (ms * 1e-3) / 1e9
-        line = {"variant": name, "n": n, "order": m, "rk": p["rk"], "limiter": p["limiter"], "sub_steps": sub,
+        line = {"variant": name, "n": n, "order": m, "rk": p["rk"], "limiter": p["limiter"], "flux": p["flux"], "sub_steps": sub,
                 "steps": steps, "ms_per_step": ms, "ms_per_sub_step": ms / sub,
                 "dof_updates_per_s": W.dof_count(p) * sub / (ms * 1e-3),
                 "launches_per_step": (g.launch_count - l0) / steps,

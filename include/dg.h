@@ -65,6 +65,8 @@ typedef struct {
                                      every RK sub-step (step (iii)(d)), and dg_cfl_dt uses the factor
                                      min(1/(2N_p+1), w_1/2) of PAPER.md:131; 0: off */
   double  lim_eps;                /* limiter floor for density and pressure (> 0 when limiter = 1; 1e-13) */
+  int32_t flux;                   /* numerical flux h_{e,K} of Eq.(3) (PAPER.md:97 leaves its type open): 0 local
+                                     Lax-Friedrichs (BASELINE cfg0); 1 HLLC (eos 0) / HLL (eos 1), Davis wave speeds */
   double  damp_in_r0, damp_in_r1; /* inner wave-killing zone of the paper's own disc: active for
                                      r < damp_in_r0 (= r_d), full strength for r <= damp_in_r1 (= r_in < r_d);
                                      damp_in_r0 <= 0: off */

@@ -39,6 +39,7 @@ bool valid_params(const dg_params* p) {
   if (!(p->x1 > p->x0) || !(p->y1 > p->y0)) return false;
   if (p->rk < 2 || p->rk > 5) return false;
   if (p->limiter != 0 && p->limiter != 1) return false;
+  if (p->flux != 0 && p->flux != 1) return false;
   if (p->limiter == 1 && !(p->lim_eps > 0.0)) return false;
   if (p->bc < 0 || p->bc > 2 || p->eos < 0 || p->eos > 1) return false;
   if (p->eos == 0 && !(p->gamma > 1.0)) return false;
@@ -218,12 +219,22 @@ int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout,
   const bool timed = c->timing && c->ev_used + 2 <= c->evs.size();
   if (timed) cudaEventRecord(c->evs[c->ev_used], c->stream);
   cudaError_t e;
-  switch (c->L.m) {
-    case 1: e = launch_stage_m1(A, c->p.eos, grav, kind, grid, c->stream); break;
-    case 2: e = launch_stage_m2(A, c->p.eos, grav, kind, grid, c->stream); break;
-    case 3: e = launch_stage_m3(A, c->p.eos, grav, kind, grid, c->stream); break;
-    case 4: e = launch_stage_m4(A, c->p.eos, grav, kind, grid, c->stream); break;
-    default: e = launch_stage_m5(A, c->p.eos, grav, kind, grid, c->stream); break;
+  if (c->p.flux == 0) {
+    switch (c->L.m) {
+      case 1: e = launch_stage_m1(A, c->p.eos, grav, kind, grid, c->stream); break;
+      case 2: e = launch_stage_m2(A, c->p.eos, grav, kind, grid, c->stream); break;
+      case 3: e = launch_stage_m3(A, c->p.eos, grav, kind, grid, c->stream); break;
+      case 4: e = launch_stage_m4(A, c->p.eos, grav, kind, grid, c->stream); break;
+      default: e = launch_stage_m5(A, c->p.eos, grav, kind, grid, c->stream); break;
+    }
+  } else {
+    switch (c->L.m) {
+      case 1: e = launch_stage_m1f(A, c->p.eos, grav, kind, grid, c->stream); break;
+      case 2: e = launch_stage_m2f(A, c->p.eos, grav, kind, grid, c->stream); break;
+      case 3: e = launch_stage_m3f(A, c->p.eos, grav, kind, grid, c->stream); break;
+      case 4: e = launch_stage_m4f(A, c->p.eos, grav, kind, grid, c->stream); break;
+      default: e = launch_stage_m5f(A, c->p.eos, grav, kind, grid, c->stream); break;
+    }
   }
   c->launches++;
   if (timed) {

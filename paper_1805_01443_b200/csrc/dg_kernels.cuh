@@ -125,6 +125,8 @@ __device__ __forceinline__ double rcp_fast(double x) {
   const double e = fma(-x, r, 1.0);             // r <- r (1 + e + e^2), e ~ 1e-6
   return fma(r, fma(e, e, e), r);
 }
+// same for either sign of x (the MUFU seed carries the sign)
+__device__ __forceinline__ double rcp_fast_signed(double x) { return copysign(rcp_fast(fabs(x)), x); }
 __device__ __forceinline__ double rsqrt_fast(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
@@ -170,6 +172,80 @@ __device__ __forceinline__ void llf2(const double (&UL)[4], const double (&FL)[4
   for (int v = 0; v < 4; ++v) H[v] = fma(-lam, UR[v] - UL[v], FL[v] + FR[v]);
 }
 
+// What a Riemann solver needs from one side of a face besides U and F.  FLUX 0 (local Lax-Friedrichs): the
+// signal speed |v_n| + c; FLUX 1 (HLLC for the ideal gas, HLL for the isothermal closure; SURVEY.md 8(f)
+// NEXT-4): normal velocity, sound speed and pressure.
+template <int FLUX> struct Wave;
+template <> struct Wave<0> { double lam; };
+template <> struct Wave<1> { double vn, c, pr; };
+
+template <int EOS, int DIR, int FLUX>
+__device__ __forceinline__ void face_flux(const Phys& ph, const double (&u)[4], double cs2, double ciso,
+                                          double (&F)[4], Wave<FLUX>& w) {
+  if constexpr (FLUX == 0) {
+    euler_flux<EOS, DIR, true>(ph, u, cs2, ciso, F, w.lam);
+  } else {
+    const double rinv = rcp_fast(u[0]);
+    const double vx = u[1] * rinv, vy = u[2] * rinv;
+    double pr;
+    if (EOS == 0) pr = ph.gm1 * (u[3] - 0.5 * fma(u[1], vx, u[2] * vy));
+    else          pr = cs2 * u[0];
+    const double vn = DIR == 0 ? vx : vy;
+    F[0] = u[1 + DIR];
+    F[1] = DIR == 0 ? fma(u[1], vn, pr) : u[1] * vn;
+    F[2] = DIR == 1 ? fma(u[2], vn, pr) : u[2] * vn;
+    F[3] = (u[3] + pr) * vn;
+    w.vn = vn;
+    w.c = EOS == 0 ? sqrt_fast(ph.gamma * pr * rinv) : ciso;
+    w.pr = pr;
+  }
+}
+
+// Numerical flux TIMES TWO through a face with normal +DIR (the 1/2 lives in the lifting tables), left state
+// first.  FLUX 1: Davis wave speeds S_L = min(v_L - c_L, v_R - c_R), S_R = max(v_L + c_L, v_R + c_R); HLL
+// (S_R F_L - S_L F_R + S_L S_R (U_R - U_L))/(S_R - S_L) for the isothermal closure; HLLC (Toro, Spruce &
+// Speares 1994) with the contact speed S* and the star state of the upwind side for the ideal gas.
+template <int FLUX, int EOS, int DIR>
+__device__ __forceinline__ void riemann2(const double (&UL)[4], const double (&FL)[4], const Wave<FLUX>& wL,
+                                         const double (&UR)[4], const double (&FR)[4], const Wave<FLUX>& wR,
+                                         double (&H)[4]) {
+  if constexpr (FLUX == 0) {
+    llf2(UL, FL, wL.lam, UR, FR, wR.lam, H);
+  } else {
+    const double SL = fmin(wL.vn - wL.c, wR.vn - wR.c), SR = fmax(wL.vn + wL.c, wR.vn + wR.c);
+    if (SL >= 0.0) {
+#pragma unroll
+      for (int v = 0; v < 4; ++v) H[v] = 2.0 * FL[v];
+    } else if (SR <= 0.0) {
+#pragma unroll
+      for (int v = 0; v < 4; ++v) H[v] = 2.0 * FR[v];
+    } else if (EOS == 1) {
+      const double k = 2.0 * rcp_fast(SR - SL);
+#pragma unroll
+      for (int v = 0; v < 4; ++v) H[v] = k * (SR * FL[v] - SL * FR[v] + SL * SR * (UR[v] - UL[v]));
+    } else {
+      constexpr int n = 1 + DIR, tg = 2 - DIR;
+      const double mL = UL[0] * (SL - wL.vn), mR = UR[0] * (SR - wR.vn);
+      const double Ss = (wR.pr - wL.pr + UL[n] * (SL - wL.vn) - UR[n] * (SR - wR.vn)) * rcp_fast_signed(mL - mR);
+      const bool left = Ss >= 0.0;
+      const double S = left ? SL : SR, vK = left ? wL.vn : wR.vn, pK = left ? wL.pr : wR.pr;
+      double U[4], F[4];
+#pragma unroll
+      for (int v = 0; v < 4; ++v) { U[v] = left ? UL[v] : UR[v]; F[v] = left ? FL[v] : FR[v]; }
+      const double rinv = rcp_fast(U[0]);
+      const double m = U[0] * (S - vK);                       // rho_K (S_K - v_K)
+      const double fac = m * rcp_fast_signed(S - Ss);
+      double Us[4];
+      Us[0] = fac;
+      Us[n] = fac * Ss;
+      Us[tg] = fac * (U[tg] * rinv);
+      Us[3] = fac * (U[3] * rinv + (Ss - vK) * (Ss + pK * rcp_fast_signed(m)));
+#pragma unroll
+      for (int v = 0; v < 4; ++v) H[v] = 2.0 * fma(S, Us[v] - U[v], F[v]);
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // Trace of a cell at eta = -1/+1 (node stride `s` doubles: 32 inside a tile)
 // ---------------------------------------------------------------------------------------------
@@ -187,6 +263,10 @@ __device__ __forceinline__ void column_trace(const double* cell, int stride, int
 
 __device__ __forceinline__ double shfl_up1(double x) { return __shfl_up_sync(FULL, x, 1); }
 __device__ __forceinline__ double shfl_dn1(double x) { return __shfl_down_sync(FULL, x, 1); }
+__device__ __forceinline__ Wave<0> shfl_dn1(const Wave<0>& w) { return Wave<0>{shfl_dn1(w.lam)}; }
+__device__ __forceinline__ Wave<1> shfl_dn1(const Wave<1>& w) {
+  return Wave<1>{shfl_dn1(w.vn), shfl_dn1(w.c), shfl_dn1(w.pr)};
+}
 
 // ---------------------------------------------------------------------------------------------
 // TMA (bulk async copy) + mbarrier helpers: one contiguous 32-cell tile per copy
@@ -247,7 +327,7 @@ constexpr size_t stage_smem_bytes() {
   return ((size_t)(NST + 1) * 4 * M * M * 32 + (size_t)M * M * 32 + (size_t)4 * M * 32) * sizeof(double) + 64;
 }
 
-template <int M, int EOS, int GRAV, int KIND, int MINB>
+template <int M, int EOS, int GRAV, int KIND, int MINB, int FLUX = 0>
 __global__ void __launch_bounds__(M * 32, MINB)
 stage_kernel(const __grid_constant__ StageArgs A) {
   constexpr bool grav = GRAV != G_NONE;
@@ -374,24 +454,25 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       cs2 = A.ph.h2gm * rsqrt_fast(fma(xq_col, xq_col, fma(yS, yS, A.ph.eps2s)));
       ciso = sqrt_fast(cs2);
     }
-    double US[4], GSo[4], lamSo, bU[4], bG[4], bLam;
+    double US[4], GSo[4], bU[4], bG[4];
+    Wave<FLUX> lamSo, bLam;
     tile_wait(1);
     column_trace<M>(tiles + BS + lane, 32, w, T.Im, US);
-    euler_flux<EOS, 1, true>(A.ph, US, cs2, ciso, GSo, lamSo);
+    face_flux<EOS, 1, FLUX>(A.ph, US, cs2, ciso, GSo, lamSo);
     if (tile_row(0) >= 0) {
       tile_wait(0);
       column_trace<M>(tiles + lane, 32, w, T.Ip, bU);
-      euler_flux<EOS, 1, true>(A.ph, bU, cs2, ciso, bG, bLam);
+      face_flux<EOS, 1, FLUX>(A.ph, bU, cs2, ciso, bG, bLam);
     } else if (g.bc == 2) {
 #pragma unroll
       for (int v = 0; v < 4; ++v) bU[v] = __ldg(A.btrS + ((size_t)(ib * 4 + v) * M + w) * 32 + lane);
-      euler_flux<EOS, 1, true>(A.ph, bU, cs2, ciso, bG, bLam);
+      face_flux<EOS, 1, FLUX>(A.ph, bU, cs2, ciso, bG, bLam);
     } else {                                     // transmissive bottom boundary
 #pragma unroll
       for (int v = 0; v < 4; ++v) { bU[v] = US[v]; bG[v] = GSo[v]; }
       bLam = lamSo;
     }
-    llf2(bU, bG, bLam, US, GSo, lamSo, HS);
+    riemann2<FLUX, EOS, 1>(bU, bG, bLam, US, GSo, lamSo, HS);
   }
   __syncthreads();                               // tile 0's slot may be refilled
 
@@ -493,10 +574,12 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           cE = sqrt_fast(cs2E);
         }
       }
-      double FWo[4], FEo[4], lamWo, lamEo;
-      euler_flux<EOS, 0, true>(A.ph, UW, cs2W, cW, FWo, lamWo);
-      euler_flux<EOS, 0, true>(A.ph, UE, cs2E, cE, FEo, lamEo);
-      double UR[4], FR[4], lamR;
+      double FWo[4], FEo[4];
+      Wave<FLUX> lamWo, lamEo;
+      face_flux<EOS, 0, FLUX>(A.ph, UW, cs2W, cW, FWo, lamWo);
+      face_flux<EOS, 0, FLUX>(A.ph, UE, cs2E, cE, FEo, lamEo);
+      double UR[4], FR[4];
+      Wave<FLUX> lamR;
 #pragma unroll
       for (int v = 0; v < 4; ++v) { UR[v] = shfl_dn1(UW[v]); FR[v] = shfl_dn1(FWo[v]); }
       lamR = shfl_dn1(lamWo);
@@ -517,14 +600,15 @@ stage_kernel(const __grid_constant__ StageArgs A) {
             for (int v = 0; v < 4; ++v) UR[v] = __ldg(A.btrE + ((size_t)j * 4 + v) * M + r);
           }
         }
-        euler_flux<EOS, 0, true>(A.ph, UR, cs2E, cE, FR, lamR);
+        face_flux<EOS, 0, FLUX>(A.ph, UR, cs2E, cE, FR, lamR);
       }
       double HE[4], HW[4];
-      llf2(UE, FEo, lamEo, UR, FR, lamR, HE);
+      riemann2<FLUX, EOS, 0>(UE, FEo, lamEo, UR, FR, lamR, HE);
 #pragma unroll
       for (int v = 0; v < 4; ++v) HW[v] = shfl_up1(HE[v]);
       if (lane == 0) {                           // left neighbour is outside this block
-        double UL[4], FL[4], lamL;
+        double UL[4], FL[4];
+        Wave<FLUX> lamL;
         if (haveL) {
 #pragma unroll
           for (int v = 0; v < 4; ++v) UL[v] = UX[v];
@@ -535,8 +619,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 #pragma unroll
           for (int v = 0; v < 4; ++v) UL[v] = __ldg(A.btrW + ((size_t)j * 4 + v) * M + r);
         }
-        euler_flux<EOS, 0, true>(A.ph, UL, cs2W, cW, FL, lamL);
-        llf2(UL, FL, lamL, UW, FWo, lamWo, HW);
+        face_flux<EOS, 0, FLUX>(A.ph, UL, cs2W, cW, FL, lamL);
+        riemann2<FLUX, EOS, 0>(UL, FL, lamL, UW, FWo, lamWo, HW);
       }
       // a u^n (landed in sN) + x-part of beta N
       if (use_un) mbar_wait(mbar + NST, (uint32_t)((t - 1) & 1));
@@ -629,13 +713,15 @@ stage_kernel(const __grid_constant__ StageArgs A) {
         cs2N = A.ph.h2gm * rsqrt_fast(fma(xq, xq, fma(yN, yN, A.ph.eps2s)));
         cN = sqrt_fast(cs2N);
       }
-      double GNo[4], lamNo;
-      euler_flux<EOS, 1, true>(A.ph, UN, cs2N, cN, GNo, lamNo);
-      double aU[4], aG[4], aLam;
+      double GNo[4];
+      Wave<FLUX> lamNo;
+      face_flux<EOS, 1, FLUX>(A.ph, UN, cs2N, cN, GNo, lamNo);
+      double aU[4], aG[4];
+      Wave<FLUX> aLam;
       if (tile_row(t + 1) >= 0) {
         tile_wait(t + 1);
         column_trace<M>(tiles + ((t + 1) % NST) * BS + lane, 32, q, T.Im, aU);
-        euler_flux<EOS, 1, true>(A.ph, aU, cs2N, cN, aG, aLam);
+        face_flux<EOS, 1, FLUX>(A.ph, aU, cs2N, cN, aG, aLam);
       } else if (g.bc == 1) {
 #pragma unroll
         for (int v = 0; v < 4; ++v) { aU[v] = UN[v]; aG[v] = GNo[v]; }
@@ -643,10 +729,10 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       } else {
 #pragma unroll
         for (int v = 0; v < 4; ++v) aU[v] = __ldg(A.btrN + ((size_t)(ib * 4 + v) * M + q) * 32 + lane);
-        euler_flux<EOS, 1, true>(A.ph, aU, cs2N, cN, aG, aLam);
+        face_flux<EOS, 1, FLUX>(A.ph, aU, cs2N, cN, aG, aLam);
       }
       double HN[4];
-      llf2(UN, GNo, lamNo, aU, aG, aLam, HN);
+      riemann2<FLUX, EOS, 1>(UN, GNo, lamNo, aU, aG, aLam, HN);
 
       // modal update in nodal form + RK combination (rows a8, a9) and store
       const size_t cell_off = j * row_stride + (size_t)ib * BS + lane;

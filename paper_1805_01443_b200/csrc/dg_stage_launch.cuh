@@ -1,5 +1,5 @@
 // Launch dispatch of the stage kernel for one DG order M: one translation unit per order
-// (dg_stage_m1.cu ... dg_stage_m5.cu) so that the 35 variants per order compile in parallel.
+// (dg_stage_m1.cu ... dg_stage_m5.cu) and numerical flux, so that the 35 variants of each compile in parallel.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -17,11 +17,11 @@ template <> struct StageMinBlocks<3> { static constexpr int value = 5; };
 template <> struct StageMinBlocks<4> { static constexpr int value = 3; };
 template <> struct StageMinBlocks<5> { static constexpr int value = 2; };
 
-template <int M, int EOS, int GRAV, int KIND>
+template <int M, int EOS, int GRAV, int KIND, int FLUX>
 cudaError_t launch_stage_variant(const StageArgs& A, dim3 grid, cudaStream_t stream) {
   static bool attr_set = false;      // dynamic shared memory above 48 KB must be opted in once
   constexpr size_t smem = stage_smem_bytes<M>();
-  auto kern = stage_kernel<M, EOS, GRAV, KIND, StageMinBlocks<M>::value>;
+  auto kern = stage_kernel<M, EOS, GRAV, KIND, StageMinBlocks<M>::value, FLUX>;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -31,38 +31,41 @@ cudaError_t launch_stage_variant(const StageArgs& A, dim3 grid, cudaStream_t str
   return cudaGetLastError();
 }
 
-template <int M, int EOS, int GRAV>
+template <int M, int EOS, int GRAV, int FLUX>
 cudaError_t launch_stage_kind(const StageArgs& A, int kind, dim3 grid, cudaStream_t s) {
   switch (kind) {
-    case K_RHS:   return launch_stage_variant<M, EOS, GRAV, K_RHS>(A, grid, s);
-    case K_FIRST: return launch_stage_variant<M, EOS, GRAV, K_FIRST>(A, grid, s);
-    case K_MID:   return launch_stage_variant<M, EOS, GRAV, K_MID>(A, grid, s);
-    case K_LAST:  return launch_stage_variant<M, EOS, GRAV, K_LAST>(A, grid, s);
-    case K_LASTD: return launch_stage_variant<M, EOS, GRAV, K_LASTD>(A, grid, s);
-    case K_GEN:   return launch_stage_variant<M, EOS, GRAV, K_GEN>(A, grid, s);
-    default:      return launch_stage_variant<M, EOS, GRAV, K_GENL>(A, grid, s);
+    case K_RHS:   return launch_stage_variant<M, EOS, GRAV, K_RHS, FLUX>(A, grid, s);
+    case K_FIRST: return launch_stage_variant<M, EOS, GRAV, K_FIRST, FLUX>(A, grid, s);
+    case K_MID:   return launch_stage_variant<M, EOS, GRAV, K_MID, FLUX>(A, grid, s);
+    case K_LAST:  return launch_stage_variant<M, EOS, GRAV, K_LAST, FLUX>(A, grid, s);
+    case K_LASTD: return launch_stage_variant<M, EOS, GRAV, K_LASTD, FLUX>(A, grid, s);
+    case K_GEN:   return launch_stage_variant<M, EOS, GRAV, K_GEN, FLUX>(A, grid, s);
+    default:      return launch_stage_variant<M, EOS, GRAV, K_GENL, FLUX>(A, grid, s);
   }
 }
 
-template <int M>
+template <int M, int FLUX>
 cudaError_t launch_stage_order(const StageArgs& A, int eos, int grav, int kind, dim3 grid, cudaStream_t s) {
   if (eos == 0) {
     switch (grav) {
-      case G_NONE: return launch_stage_kind<M, 0, G_NONE>(A, kind, grid, s);
-      case G_STAR: return launch_stage_kind<M, 0, G_STAR>(A, kind, grid, s);
-      default:     return launch_stage_kind<M, 0, G_PLANET>(A, kind, grid, s);
+      case G_NONE: return launch_stage_kind<M, 0, G_NONE, FLUX>(A, kind, grid, s);
+      case G_STAR: return launch_stage_kind<M, 0, G_STAR, FLUX>(A, kind, grid, s);
+      default:     return launch_stage_kind<M, 0, G_PLANET, FLUX>(A, kind, grid, s);
     }
   }
   // the locally isothermal closure is defined through the star (c_s^2 ~ GM/r): gravity is always on
-  if (grav == G_PLANET) return launch_stage_kind<M, 1, G_PLANET>(A, kind, grid, s);
-  return launch_stage_kind<M, 1, G_STAR>(A, kind, grid, s);
+  if (grav == G_PLANET) return launch_stage_kind<M, 1, G_PLANET, FLUX>(A, kind, grid, s);
+  return launch_stage_kind<M, 1, G_STAR, FLUX>(A, kind, grid, s);
 }
 
-// one definition per order, in dg_stage_m<M>.cu
-cudaError_t launch_stage_m1(const StageArgs&, int eos, int grav, int kind, dim3 grid, cudaStream_t);
-cudaError_t launch_stage_m2(const StageArgs&, int eos, int grav, int kind, dim3 grid, cudaStream_t);
-cudaError_t launch_stage_m3(const StageArgs&, int eos, int grav, int kind, dim3 grid, cudaStream_t);
-cudaError_t launch_stage_m4(const StageArgs&, int eos, int grav, int kind, dim3 grid, cudaStream_t);
-cudaError_t launch_stage_m5(const StageArgs&, int eos, int grav, int kind, dim3 grid, cudaStream_t);
+// one definition per order and numerical flux (0: local Lax-Friedrichs, 1: HLLC / HLL), in dg_stage_m<M>.cu
+// and dg_stage_m<M>f.cu
+#define DG_DECLARE_STAGE(name) \
+  cudaError_t name(const StageArgs&, int eos, int grav, int kind, dim3 grid, cudaStream_t)
+DG_DECLARE_STAGE(launch_stage_m1); DG_DECLARE_STAGE(launch_stage_m2); DG_DECLARE_STAGE(launch_stage_m3);
+DG_DECLARE_STAGE(launch_stage_m4); DG_DECLARE_STAGE(launch_stage_m5);
+DG_DECLARE_STAGE(launch_stage_m1f); DG_DECLARE_STAGE(launch_stage_m2f); DG_DECLARE_STAGE(launch_stage_m3f);
+DG_DECLARE_STAGE(launch_stage_m4f); DG_DECLARE_STAGE(launch_stage_m5f);
+#undef DG_DECLARE_STAGE
 
 }  // namespace dg

@@ -1,0 +1,7 @@
+// Stage-kernel variants of DG order 4, HLLC / HLL flux (see dg_stage_launch.cuh).
+#include "dg_stage_launch.cuh"
+namespace dg {
+cudaError_t launch_stage_m4f(const StageArgs& A, int eos, int grav, int kind, dim3 grid, cudaStream_t s) {
+  return launch_stage_order<4, 1>(A, eos, grav, kind, grid, s);
+}
+}  // namespace dg

@@ -35,6 +35,7 @@ class DGParams(C.Structure):
         ("omega_planet", C.c_double), ("phase0", C.c_double),
         ("damp_r0", C.c_double), ("damp_r1", C.c_double), ("t0", C.c_double),
         ("limiter", C.c_int32), ("lim_eps", C.c_double),
+        ("flux", C.c_int32),
         ("damp_in_r0", C.c_double), ("damp_in_r1", C.c_double),
     ]
 

@@ -483,3 +483,53 @@ def test_full_size_next_rows(DG):
     assert abs(g.cfl_dt(0.2) / ref.cfl_dt(0.2) - 1.0) < 1e-12
     gr = ref.torque(ref.time)
     assert abs(g.torque(ref.time) - gr) < 1e-11 * max(1.0, abs(gr))
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-4: HLLC (ideal gas) / HLL (isothermal) flux option
+@pytest.mark.parametrize("rk", [3, 5])
+@pytest.mark.parametrize("case", NEXT_CASES + [dict(nx=1, ny=1, m=4, eos=0, bc=0, gravity=False)], ids=_id)
+def test_hllc_parity(DG, case, rk):
+    p, U = _make(case, rk=rk, seed=13)
+    p["flux"] = 1
+    if case["eos"] == 1:
+        p["damp_r0"], p["damp_r1"] = 0.6, 1.2
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    g = DG(p)
+    g.set_tuning(1, 4)
+    g.set_state(dev(U))
+    dt = ref.cfl_dt(0.2)
+    L = g.rhs(0.21).cpu().numpy()
+    assert rhs_effect_err(L, ref.rhs(0.21), U, dt) < TOL_STAGE
+    st_ref = ref.step_debug(dt)
+    st = g.step_debug(dt).cpu().numpy()
+    for s in range(st.shape[0]):
+        assert rel_err(st[s], st_ref[s]) < TOL_STAGE, f"sub-step {s + 1}"
+    g2 = DG(p)
+    g2.set_state(dev(U))
+    g2.step(dt)
+    assert rel_err(g2.get_state().cpu().numpy(), ref.get_state()) < TOL_STAGE
+    # a different operator from the LLF one
+    g3 = DG(dict(p, flux=0))
+    g3.set_state(dev(U))
+    if case["m"] > 1 and case["nx"] > 1:
+        assert np.abs(g3.rhs(0.21).cpu().numpy() - L).max() > 1e-6
+
+
+def test_hllc_100_steps_and_conservation(DG):
+    p, U = W.vortex(32, 3, rk=3)
+    p["flux"] = 1
+    assert _run_100(DG, p, U) < TOL_100
+    p, U = W.disc(64, 4, planet=True, noise=1e-4)
+    p["flux"] = 1                                          # HLL with the isothermal closure
+    assert _run_100(DG, p, U) < TOL_100
+    p, U = W.random_smooth(70, 20, 4, seed=9, bc=0, rk=3)
+    p["flux"] = 1
+    g = DG(p)
+    g.set_state(dev(U))
+    tot0 = U[..., 0, 0].sum(axis=(0, 1))
+    for _ in range(10):
+        g.step(g.cfl_dt(0.2))
+    tot1 = g.get_state().cpu().numpy()[..., 0, 0].sum(axis=(0, 1))
+    assert (np.abs(tot1 - tot0) / np.abs(U[..., 0, 0]).sum(axis=(0, 1))).max() < 5e-15
