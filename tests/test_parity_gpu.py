@@ -533,3 +533,29 @@ def test_hllc_100_steps_and_conservation(DG):
         g.step(g.cfl_dt(0.2))
     tot1 = g.get_state().cpu().numpy()[..., 0, 0].sum(axis=(0, 1))
     assert (np.abs(tot1 - tot0) / np.abs(U[..., 0, 0]).sum(axis=(0, 1))).max() < 5e-15
+
+
+def test_literal_baseline_disc_runs_with_the_limiter(DG):
+    """BASELINE.json configs[1] with its literal numbers (floor 1e-6, star softening 0.02, 256^2, order 3, 200
+    steps): without the limiter the density goes negative before step 200, with it the run completes with
+    every nodal density positive -- the reason the default recipe deviates is gone once
+    `limiter = 1`."""
+    p, U = W.disc(256, 3, **W.LITERAL_BASELINE_DISC)
+    g = DG(dict(p, limiter=1))
+    g.set_state(dev(U))
+    g.limit()
+    for _ in range(200):
+        g.step(g.cfl_dt(0.2))
+    S = g.get_state().cpu().numpy()
+    assert np.isfinite(S).all() and W.evaluate_nodal(p, S)[:, :, 0].min() > 0
+    g0 = DG(p)
+    g0.set_state(dev(U))
+    bad = False
+    for _ in range(200):
+        dt = g0.cfl_dt(0.2)
+        if not (np.isfinite(dt) and dt > 0):
+            bad = True
+            break
+        g0.step(dt)
+    S0 = g0.get_state().cpu().numpy()
+    assert bad or not np.isfinite(S0).all() or W.evaluate_nodal(p, S0)[:, :, 0].min() < 0
