@@ -70,6 +70,10 @@ typedef struct {
   double  damp_in_r0, damp_in_r1; /* inner wave-killing zone of the paper's own disc: active for
                                      r < damp_in_r0 (= r_d), full strength for r <= damp_in_r1 (= r_in < r_d);
                                      damp_in_r0 <= 0: off */
+  int32_t halo_south, halo_north; /* 1: this context is one strip of a domain decomposed along y (the paper's
+                                     one-sub-domain-per-GPU design): the rows below y0 / above y1
+                                     belong to a neighbour strip and are read from a halo row the caller fills before
+                                     every sub-step (dg_halo_layout), instead of applying `bc` at that edge */
 } dg_params;
 
 /* Bytes of DEVICE workspace dg_init needs for these parameters (0 if they are invalid). */
@@ -106,6 +110,21 @@ int dg_cfl_dt(dg_ctx*, double cfl, double* dt /*HOST*/);
  * u^(s) = alpha_s u^n + beta_s (u^(s-1) + dt L(u^(s-1), t^n + c_s dt)), then the wave-killing
  * relaxation Q <- (dt Q0 + tau Q)/(tau + dt) if enabled; t += dt. */
 int dg_step(dg_ctx*, double dt);
+
+/* The same step, one sub-step at a time, for strips of a decomposed domain ("one layer of ghost
+ * cells per side", exchanged after every sub-step): dg_step_begin(dt); then k = dg_rk_stages(rk) times
+ * { fill the halo rows; dg_substep(); }; then dg_step_end().  dg_step is exactly this sequence. */
+int dg_step_begin(dg_ctx*, double dt);
+int dg_substep(dg_ctx*);
+int dg_step_end(dg_ctx*);
+
+/* Where the halo exchange reads and writes, as byte offsets into the workspace given to dg_init (internal
+ * layout, one row of cells = *row_bytes contiguous bytes): offsets[0], [1] = first and last row of the array
+ * the next stage kernel reads (the next sub-step's input inside a split step, else the current state; the same
+ * for dg_rhs): what the south / north neighbour needs; offsets[2], [3] = this context's south / north halo row
+ * ((size_t)-1 if that edge is a domain boundary).  The caller copies neighbour rows into the halo rows on the
+ * context's stream (cudaMemcpyAsync, NCCL send/recv, or a peer-to-peer copy over NVLink). */
+int dg_halo_layout(dg_ctx*, size_t offsets[4] /*HOST*/, size_t* row_bytes /*HOST*/);
 
 /* Same, and also writes the results of the k = dg_rk_stages(rk) sub-steps (after the limiter, before
  * damping; the last one is u^{n+1}), modal layout, stages: [k][ny][nx][4][m][m] DEVICE.  For per-stage

@@ -29,6 +29,8 @@ struct Layout {
   size_t state_bytes;
   bool need_q0, need_btr;
   int nkbuf;                 // slope buffers K_j of the Butcher-form schemes (rk 4: 4, rk 5: 5)
+  size_t row_bytes;          // one row of tiles: nbx * 4 m^2 * 32 doubles
+  size_t off_haloS, off_haloN;
   size_t off_q[3], off_k[MAXK], off_q0, off_btrW, off_btrE, off_btrS, off_btrN, off_partial, off_scalars, total;
 };
 
@@ -41,6 +43,7 @@ bool valid_params(const dg_params* p) {
   if (p->rk < 2 || p->rk > 5) return false;
   if (p->limiter != 0 && p->limiter != 1) return false;
   if (p->flux != 0 && p->flux != 1) return false;
+  if ((p->halo_south != 0 && p->halo_south != 1) || (p->halo_north != 0 && p->halo_north != 1)) return false;
   if (p->limiter == 1 && !(p->lim_eps > 0.0)) return false;
   if (p->bc < 0 || p->bc > 2 || p->eos < 0 || p->eos > 1) return false;
   if (p->eos == 0 && !(p->gamma > 1.0)) return false;
@@ -72,6 +75,9 @@ Layout make_layout(const dg_params* p) {
   L.off_btrE = off; if (L.need_btr) off += side;
   L.off_btrS = off; if (L.need_btr) off += top;
   L.off_btrN = off; if (L.need_btr) off += top;
+  L.row_bytes = (size_t)L.nbx * 4 * L.m * L.m * 32 * sizeof(double);
+  L.off_haloS = off; if (p->halo_south) off += align_up(L.row_bytes);
+  L.off_haloN = off; if (p->halo_north) off += align_up(L.row_bytes);
   // torque partial sums: 2 doubles per block of torque_kernel
   L.off_partial = off; off += align_up((size_t)L.nbx * ((p->ny + 3) / 4) * 2 * sizeof(double));
   L.off_scalars = off; off += ALIGN;
@@ -98,6 +104,10 @@ struct dg_ctx {
   int rows_per_cta;
   int fused_cfl;
   int gen_pf;
+  bool step_active;           // between dg_step_begin and dg_step_end
+  int step_next;              // next sub-step of the split step
+  double step_dt;
+  int step_A;
   long long launches;
   bool timing;
   std::vector<cudaEvent_t> evs;      // pairs (start, stop) around stage kernels, recorded without syncing
@@ -107,6 +117,8 @@ struct dg_ctx {
   double* q(int k) const { return reinterpret_cast<double*>(ws + L.off_q[k]); }
   double* kbuf(int k) const { return reinterpret_cast<double*>(ws + L.off_k[k]); }
   double* partial() const { return reinterpret_cast<double*>(ws + L.off_partial); }
+  double* haloS() const { return p.halo_south ? reinterpret_cast<double*>(ws + L.off_haloS) : nullptr; }
+  double* haloN() const { return p.halo_north ? reinterpret_cast<double*>(ws + L.off_haloN) : nullptr; }
   double* q0() const { return reinterpret_cast<double*>(ws + L.off_q0); }
   double* btrW() const { return reinterpret_cast<double*>(ws + L.off_btrW); }
   double* btrE() const { return reinterpret_cast<double*>(ws + L.off_btrE); }
@@ -204,6 +216,7 @@ int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout,
   }
   A.qprev = qprev; A.qn = qn; A.qout = qout; A.q0 = c->q0();
   A.btrW = c->btrW(); A.btrE = c->btrE(); A.btrS = c->btrS(); A.btrN = c->btrN();
+  A.haloS = c->haloS(); A.haloN = c->haloN();
   A.wmax = c->wmax();
   A.a = a; A.b = b; A.dt = dt;
   A.D = make_damp(c, dt);
@@ -371,69 +384,93 @@ int launch_limit(dg_ctx* c, double* Q, bool final_, double dt) {
 // relaxation and the CFL reduction for the next step ride on the last kernel of the step: the last
 // stage kernel (limiter off) or the last limiter pass (limiter on).  With `stages` (debug path) they
 // run as their own passes so that the recorded sub-step results are "before damping".
-int do_step(dg_ctx* c, double dt, double* stages) {
-  if (!c) return DG_EINVAL;
-  if (!c->has_state) return fail(c, DG_ESTATE, "dg_step: state not set");
-  if (!(dt >= 0.0) || !std::isfinite(dt)) return fail(c, DG_EINVAL, "dg_step: bad dt");
-  const int A = c->cur, B = (c->cur + 1) % 3, Cc = (c->cur + 2) % 3;
-  const size_t n = (size_t)c->p.ny * c->p.nx * 4 * c->L.m * c->L.m;
-  const bool damp = has_damping(c->p);
-  const bool lim = c->p.limiter != 0;
-  const bool fuse_tail = !stages && (c->fused_cfl || damp);   // damping + CFL ride on the step's last kernel
+// Buffers of sub-step i of a step that started with u^n in buffer A: reads in(i), writes out(i).
+inline int substep_out(int A, int i) { return (A + 1 + (i & 1)) % 3; }
+inline int substep_in(int A, int i) { return i == 0 ? A : substep_out(A, i - 1); }
+
+struct StepPlan { int A, k; bool damp, lim, fuse_tail; double dt; double* stages; };
+
+StepPlan make_plan(const dg_ctx* c, double dt, double* stages) {
+  StepPlan P{};
+  P.A = c->cur;
+  P.k = dg_rk_stages(c->p.rk);
+  P.damp = has_damping(c->p);
+  P.lim = c->p.limiter != 0;
+  P.fuse_tail = !stages && (c->fused_cfl || P.damp);   // damping + CFL ride on the step's last kernel
+  P.dt = dt;
+  P.stages = stages;
+  return P;
+}
+
+int step_begin(dg_ctx* c, const StepPlan& P) {
+  if (P.fuse_tail) CUDA_TRY(c, cudaMemsetAsync(c->wmax(), 0, sizeof(unsigned long long), c->stream));
+  return DG_OK;
+}
+
+// Sub-step i: one fused stage kernel, then the limiter when it is on, then (debug) the copy-out.
+int run_substep(dg_ctx* c, const StepPlan& P, int i) {
+  const double dt = P.dt;
+  const bool last = i + 1 == P.k;
+  const double* qin = c->q(substep_in(P.A, i));
+  const double* qn = c->q(P.A);
+  double* qout = c->q(substep_out(P.A, i));
   int e;
-  if (fuse_tail) CUDA_TRY(c, cudaMemsetAsync(c->wmax(), 0, sizeof(unsigned long long), c->stream));
-  // after every sub-step: limiter, then (debug) the copy-out
-  auto after = [&](double* Q, int k, bool last) -> int {
-    int err = DG_OK;
-    if (lim) err = launch_limit(c, Q, last && fuse_tail, dt);
-    if (!err && stages) err = to_modal(c, Q, stages + (size_t)k * n);
-    return err;
-  };
   if (c->p.rk <= 3) {
     // SSP-RK in Shu-Osher form, stage times c = (0,1) / (0,1,1/2)
-    const int last = (fuse_tail && !lim) ? (damp ? K_LASTD : K_LAST) : K_MID;
-    if ((e = launch_stage(c, c->q(A), c->q(A), c->q(B), 0.0, 1.0, dt, c->t, K_FIRST))) return e;
-    if ((e = after(c->q(B), 0, false))) return e;
-    if (c->p.rk == 2) {
-      if ((e = launch_stage(c, c->q(B), c->q(A), c->q(Cc), 0.5, 0.5, dt, c->t + dt, last))) return e;
-      if ((e = after(c->q(Cc), 1, true))) return e;
-      c->cur = Cc;
-    } else {
-      if ((e = launch_stage(c, c->q(B), c->q(A), c->q(Cc), 0.75, 0.25, dt, c->t + dt, K_MID))) return e;
-      if ((e = after(c->q(Cc), 1, false))) return e;
-      if ((e = launch_stage(c, c->q(Cc), c->q(A), c->q(B), 1.0 / 3.0, 2.0 / 3.0, dt, c->t + 0.5 * dt, last))) return e;
-      if ((e = after(c->q(B), 2, true))) return e;
-      c->cur = B;
-    }
+    const int last_kind = (P.fuse_tail && !P.lim) ? (P.damp ? K_LASTD : K_LAST) : K_MID;
+    if (i == 0)                  e = launch_stage(c, qin, qn, qout, 0.0, 1.0, dt, c->t, K_FIRST);
+    else if (c->p.rk == 2)       e = launch_stage(c, qin, qn, qout, 0.5, 0.5, dt, c->t + dt, last_kind);
+    else if (i == 1)             e = launch_stage(c, qin, qn, qout, 0.75, 0.25, dt, c->t + dt, K_MID);
+    else                         e = launch_stage(c, qin, qn, qout, 1.0 / 3.0, 2.0 / 3.0, dt, c->t + 0.5 * dt, last_kind);
   } else {
     // Butcher form (Appendix A): y_{i+1} = u^n + sum_{j<=i} a_{i+1,j} K_j, K_j = dt N(y_j, t_j),
     // the last row being b.  Sub-step i reads y_i (with halo), u^n and the earlier K_j, writes K_i and y_{i+1}.
     ButcherTableau bt;
     butcher_tableau(c->p.rk, &bt);
-    int in = A, out = B;
-    for (int i = 0; i < bt.s; ++i) {
-      const bool last = i + 1 == bt.s;
-      const double* coef = last ? bt.b : bt.a[i + 1];
-      GenArgs ga{};
-      for (int j = 0; j < i; ++j)
-        if (coef[j] != 0.0) { ga.kin[ga.nk] = c->kbuf(j); ga.kc[ga.nk] = coef[j]; ga.nk++; }
-      ga.kself = coef[i];
-      ga.kout = last ? nullptr : c->kbuf(i);
-      const int kind = (last && fuse_tail && !lim) ? K_GENL : K_GEN;
-      // without the fused tail K_GENL must not damp: K_GEN never does
-      if ((e = launch_stage(c, c->q(in), c->q(A), c->q(out), 0.0, 0.0, dt, c->t + bt.c[i] * dt, kind, &ga))) return e;
-      if ((e = after(c->q(out), i, last))) return e;
-      in = out;
-      out = (out == B) ? Cc : B;
-    }
-    c->cur = in;
+    const double* coef = last ? bt.b : bt.a[i + 1];
+    GenArgs ga{};
+    for (int j = 0; j < i; ++j)
+      if (coef[j] != 0.0) { ga.kin[ga.nk] = c->kbuf(j); ga.kc[ga.nk] = coef[j]; ga.nk++; }
+    ga.kself = coef[i];
+    ga.kout = last ? nullptr : c->kbuf(i);
+    // K_GENL fuses wave-killing + CFL; K_GEN never damps
+    const int kind = (last && P.fuse_tail && !P.lim) ? K_GENL : K_GEN;
+    e = launch_stage(c, qin, qn, qout, 0.0, 0.0, dt, c->t + bt.c[i] * dt, kind, &ga);
   }
-  c->wmax_valid = fuse_tail && c->fused_cfl;
-  if (!fuse_tail && damp) {   // damping as its own pass (debug path, or nothing to ride on)
-    if ((e = launch_damp(c, c->q(c->cur), dt))) return e;
+  if (e) return e;
+  if (P.lim && (e = launch_limit(c, qout, last && P.fuse_tail, dt))) return e;
+  if (P.stages) {
+    const size_t n = (size_t)c->p.ny * c->p.nx * 4 * c->L.m * c->L.m;
+    if ((e = to_modal(c, qout, P.stages + (size_t)i * n))) return e;
   }
-  c->t += dt;
   return DG_OK;
+}
+
+int step_end(dg_ctx* c, const StepPlan& P) {
+  c->cur = substep_out(P.A, P.k - 1);
+  c->wmax_valid = P.fuse_tail && c->fused_cfl;
+  if (!P.fuse_tail && P.damp) {   // damping as its own pass (debug path, or nothing to ride on)
+    int e = launch_damp(c, c->q(c->cur), P.dt);
+    if (e) return e;
+  }
+  c->t += P.dt;
+  return DG_OK;
+}
+
+// One time step.  Sub-step results are limited when the limiter is on; the wave-killing
+// relaxation and the CFL reduction for the next step ride on the last kernel of the step: the last
+// stage kernel (limiter off) or the last limiter pass (limiter on).  With `stages` (debug path) they
+// run as their own passes so that the recorded sub-step results are "before damping".
+int do_step(dg_ctx* c, double dt, double* stages) {
+  if (!c) return DG_EINVAL;
+  if (!c->has_state) return fail(c, DG_ESTATE, "dg_step: state not set");
+  if (!(dt >= 0.0) || !std::isfinite(dt)) return fail(c, DG_EINVAL, "dg_step: bad dt");
+  if (c->step_active) return fail(c, DG_ESTATE, "dg_step: a split step (dg_step_begin) is in progress");
+  const StepPlan P = make_plan(c, dt, stages);
+  int e = step_begin(c, P);
+  for (int i = 0; !e && i < P.k; ++i) e = run_substep(c, P, i);
+  if (!e) e = step_end(c, P);
+  return e;
 }
 
 }  // namespace
@@ -474,6 +511,8 @@ int dg_init(const dg_params* p, void* workspace, size_t ws_bytes, void* cuda_str
     c->rows_per_cta = (int)std::max(4L, std::min(16L, rows));
   }
   c->fused_cfl = 1;
+  c->step_active = false;
+  c->step_next = 0;
   c->gen_pf = 3;
   c->launches = 0;
   c->timing = false;
@@ -619,6 +658,55 @@ int dg_torque(dg_ctx* c, double t, double* gamma_z) {
 }
 
 int dg_step(dg_ctx* c, double dt) { return do_step(c, dt, nullptr); }
+
+int dg_step_begin(dg_ctx* c, double dt) {
+  if (!c) return DG_EINVAL;
+  if (!c->has_state) return fail(c, DG_ESTATE, "dg_step_begin: state not set");
+  if (!(dt >= 0.0) || !std::isfinite(dt)) return fail(c, DG_EINVAL, "dg_step_begin: bad dt");
+  if (c->step_active) return fail(c, DG_ESTATE, "dg_step_begin: a split step is already in progress");
+  const StepPlan P = make_plan(c, dt, nullptr);
+  int e = step_begin(c, P);
+  if (e) return e;
+  c->step_active = true;
+  c->step_next = 0;
+  c->step_dt = dt;
+  c->step_A = P.A;
+  return DG_OK;
+}
+
+int dg_substep(dg_ctx* c) {
+  if (!c) return DG_EINVAL;
+  if (!c->step_active) return fail(c, DG_ESTATE, "dg_substep: no split step in progress");
+  StepPlan P = make_plan(c, c->step_dt, nullptr);
+  P.A = c->step_A;
+  if (c->step_next >= P.k) return fail(c, DG_ESTATE, "dg_substep: all sub-steps of this step have run");
+  int e = run_substep(c, P, c->step_next);
+  if (!e) c->step_next++;
+  return e;
+}
+
+int dg_step_end(dg_ctx* c) {
+  if (!c) return DG_EINVAL;
+  if (!c->step_active) return fail(c, DG_ESTATE, "dg_step_end: no split step in progress");
+  StepPlan P = make_plan(c, c->step_dt, nullptr);
+  P.A = c->step_A;
+  if (c->step_next != P.k) return fail(c, DG_ESTATE, "dg_step_end: sub-steps are missing");
+  c->step_active = false;
+  return step_end(c, P);
+}
+
+int dg_halo_layout(dg_ctx* c, size_t offsets[4], size_t* row_bytes) {
+  if (!c || !offsets || !row_bytes) return c ? fail(c, DG_EINVAL, "dg_halo_layout: null") : DG_EINVAL;
+  if (!c->has_state) return fail(c, DG_ESTATE, "dg_halo_layout: state not set");
+  // the array the next stage kernel reads: the sub-step's input inside a split step, else the current state
+  const int buf = c->step_active ? substep_in(c->step_A, c->step_next) : c->cur;
+  *row_bytes = c->L.row_bytes;
+  offsets[0] = c->L.off_q[buf];                                                 // first row: the south neighbour's north halo
+  offsets[1] = c->L.off_q[buf] + (size_t)(c->p.ny - 1) * c->L.row_bytes;          // last row: the north neighbour's south halo
+  offsets[2] = c->p.halo_south ? c->L.off_haloS : (size_t)-1;
+  offsets[3] = c->p.halo_north ? c->L.off_haloN : (size_t)-1;
+  return DG_OK;
+}
 int dg_step_debug(dg_ctx* c, double dt, double* stages) {
   if (!stages) return c ? fail(c, DG_EINVAL, "dg_step_debug: null") : DG_EINVAL;
   return do_step(c, dt, stages);

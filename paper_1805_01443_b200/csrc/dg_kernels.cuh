@@ -98,6 +98,8 @@ struct StageArgs {
   double* qout;               // u^(s)   (or N when F_RHS_ONLY)
   const double* q0;           // initial state (damping)
   const double* btrW; const double* btrE; const double* btrS; const double* btrN;  // bc 2 traces
+  const double* haloS; const double* haloN;   // strip decomposition along y: the neighbour strips' boundary rows
+                                              // of the array qprev ([nbx][4 M^2 x 32], same layout), or null
   unsigned long long* wmax;   // CFL wave-speed maximum (bit pattern of a non-negative double)
   double a, b, dt;            // out = a u^n + b u^(s-1) + beta N; beta = b dt is folded into T and ph
   DampArgs D;
@@ -376,26 +378,28 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     if (ic >= 0) edge_src = A.qprev + (size_t)(ic >> 5) * BS + (ic & 31) + (size_t)(((lane & 3) * M + w) * M) * 32;
   }
 
-  // tile t holds row j0-1+t (wrapped for periodic domains; absent outside a non-periodic domain)
+  // tile t holds row j0-1+t: wrapped for periodic domains; the neighbour strip's row (-2 south, -3 north) when
+  // the domain is one strip of a decomposition along y; absent (-1) outside a non-periodic domain
   auto tile_row = [&](int t) -> int {
     const int jj = j0 - 1 + t;
-    if (jj < 0) return g.bc == 0 ? g.ny - 1 : -1;
-    if (jj >= g.ny) return g.bc == 0 ? 0 : -1;
+    if (jj < 0) return A.haloS ? -2 : (g.bc == 0 ? g.ny - 1 : -1);
+    if (jj >= g.ny) return A.haloN ? -3 : (g.bc == 0 ? 0 : -1);
     return jj;
   };
   auto tile_issue = [&](int t) {                 // thread 0 only
     const int jr = tile_row(t);
-    if (jr >= 0) {
+    if (jr != -1) {
       uint64_t* bar = mbar + t % NST;
+      const double* src = jr >= 0 ? A.qprev + jr * row_stride : (jr == -2 ? A.haloS : A.haloN);
       mbar_expect_tx(bar, TILE_BYTES);
-      bulk_g2s(tiles + (t % NST) * BS, A.qprev + jr * row_stride + (size_t)ib * BS, TILE_BYTES, bar);
+      bulk_g2s(tiles + (t % NST) * BS, src + (size_t)ib * BS, TILE_BYTES, bar);
     }
   };
   // k-th copy into a slot completes mbarrier phase k; tile 0 is the only one that can be absent
   // and still be followed by later copies into its slot (non-periodic bottom row)
-  const int skip0 = tile_row(0) < 0 ? 1 : 0;
+  const int skip0 = tile_row(0) == -1 ? 1 : 0;
   auto tile_wait = [&](int t) {
-    if (tile_row(t) >= 0) mbar_wait(mbar + t % NST, (uint32_t)((t / NST - (t % NST == 0 ? skip0 : 0)) & 1));
+    if (tile_row(t) != -1) mbar_wait(mbar + t % NST, (uint32_t)((t / NST - (t % NST == 0 ? skip0 : 0)) & 1));
   };
   auto un_issue = [&](int j) {                   // thread 0 only; u^n tile of row j -> sN
     mbar_expect_tx(mbar + NST, TILE_BYTES);
@@ -459,7 +463,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     tile_wait(1);
     column_trace<M>(tiles + BS + lane, 32, w, T.Im, US);
     face_flux<EOS, 1, FLUX>(A.ph, US, cs2, ciso, GSo, lamSo);
-    if (tile_row(0) >= 0) {
+    if (tile_row(0) != -1) {
       tile_wait(0);
       column_trace<M>(tiles + lane, 32, w, T.Ip, bU);
       face_flux<EOS, 1, FLUX>(A.ph, bU, cs2, ciso, bG, bLam);
@@ -718,7 +722,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       face_flux<EOS, 1, FLUX>(A.ph, UN, cs2N, cN, GNo, lamNo);
       double aU[4], aG[4];
       Wave<FLUX> aLam;
-      if (tile_row(t + 1) >= 0) {
+      if (tile_row(t + 1) != -1) {
         tile_wait(t + 1);
         column_trace<M>(tiles + ((t + 1) % NST) * BS + lane, 32, q, T.Im, aU);
         face_flux<EOS, 1, FLUX>(A.ph, aU, cs2N, cN, aG, aLam);

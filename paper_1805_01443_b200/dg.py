@@ -16,6 +16,7 @@ EXPORTS = [
     "dg_time", "dg_set_time", "dg_launch_count", "dg_set_tuning", "dg_stage_timing",
     "dg_stage_time_ms", "dg_stage_times_ms", "dg_probe_fp64_peak", "dg_last_error", "dg_destroy",
     "dg_rk_stages", "dg_limit", "dg_torque",
+    "dg_step_begin", "dg_substep", "dg_step_end", "dg_halo_layout",
 ]
 
 
@@ -37,6 +38,7 @@ class DGParams(C.Structure):
         ("limiter", C.c_int32), ("lim_eps", C.c_double),
         ("flux", C.c_int32),
         ("damp_in_r0", C.c_double), ("damp_in_r1", C.c_double),
+        ("halo_south", C.c_int32), ("halo_north", C.c_int32),
     ]
 
 
@@ -80,6 +82,8 @@ def load_library(path: str | None = None):
         "dg_probe_fp64_peak": (i, [vp, C.POINTER(d)]),
         "dg_last_error": (C.c_char_p, [vp]),
         "dg_destroy": (None, [vp]),
+        "dg_step_begin": (i, [vp, d]), "dg_substep": (i, [vp]), "dg_step_end": (i, [vp]),
+        "dg_halo_layout": (i, [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
         "dg_rk_stages": (i, [i]), "dg_limit": (i, [vp]), "dg_torque": (i, [vp, d, C.POINTER(d)]),
     }
     for name, (res, args) in sig.items():
@@ -183,6 +187,34 @@ class DG:
         out = self.new_device_state((rk,)) if out is None else out
         self._chk(self.L.dg_step_debug(self._h, float(dt), self._dev(out, rk * self.ncoef)), "dg_step_debug")
         return out
+
+    def step_begin(self, dt: float):
+        self._chk(self.L.dg_step_begin(self._h, float(dt)), "dg_step_begin")
+
+    def substep(self):
+        self._chk(self.L.dg_substep(self._h), "dg_substep")
+
+    def step_end(self):
+        self._chk(self.L.dg_step_end(self._h), "dg_step_end")
+
+    @property
+    def rk_stages(self) -> int:
+        return int(self.L.dg_rk_stages(int(self.params["rk"])))
+
+    def halo_rows(self):
+        """Views into the workspace (flat fp64 tensors, internal layout): (first row, last row) of the array the
+        next stage kernel reads, and (south halo, north halo) (None at a domain boundary)."""
+        off = (C.c_size_t * 4)()
+        nb = C.c_size_t()
+        self._chk(self.L.dg_halo_layout(self._h, off, C.byref(nb)), "dg_halo_layout")
+        base = self._ws_ptr - self.workspace.data_ptr()
+
+        def view(o):
+            if o == C.c_size_t(-1).value:
+                return None
+            return self.workspace[base + o: base + o + nb.value].view(self._torch.float64)
+
+        return (view(off[0]), view(off[1])), (view(off[2]), view(off[3]))
 
     def limit(self):
         self._chk(self.L.dg_limit(self._h), "dg_limit")

@@ -37,6 +37,7 @@ _PARAM_DEFAULTS = dict(
     damp_r0=0.0, damp_r1=0.0, t0=0.0,
     limiter=0, lim_eps=1e-13, flux=0,
     damp_in_r0=0.0, damp_in_r1=0.0,
+    halo_south=0, halo_north=0,
 )
 
 

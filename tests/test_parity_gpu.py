@@ -559,3 +559,64 @@ def test_literal_baseline_disc_runs_with_the_limiter(DG):
         g0.step(dt)
     S0 = g0.get_state().cpu().numpy()
     assert bad or not np.isfinite(S0).all() or W.evaluate_nodal(p, S0)[:, :, 0].min() < 0
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-4: strips of a domain decomposed along y, halo rows exchanged before every sub-step
+@pytest.mark.parametrize("name,n_strips", [("vortex", 2), ("vortex", 3), ("disc", 4), ("disc_rk5_lim", 3), ("hllc", 2)])
+def test_strip_decomposition_reproduces_the_undivided_domain(DG, name, n_strips):
+    """All strips on one GPU (`strips.LocalStrips`): the stage kernels read the neighbour strip's boundary rows
+    from their halo rows.  Grids and boxes with binary-exact spacings, so the strips' node coordinates are the
+    undivided domain's to the last bit and the comparison is bitwise; dt (min over strips) as well."""
+    from paper_1805_01443_b200 import strips
+    if name == "vortex":
+        p, U = W.vortex(32, 3, rk=3)
+        p.update(x1=8.0, y1=8.0)                           # dx = 1/4: exact
+    elif name == "disc":
+        p, U = W.disc(64, 4, planet=True, noise=1e-4, half_width=2.0)
+    elif name == "disc_rk5_lim":
+        p, U = W.disc(64, 3, planet=True, noise=1e-4, half_width=2.0, rk=5)
+        p.update(limiter=1, damp_in_r0=0.5, damp_in_r1=0.4)
+    else:
+        p, U = W.random_smooth(40, 32, 3, seed=17, bc=1, rk=2, gravity=False)
+        p.update(flux=1, y1=2.0)
+    one = DG(p)
+    one.set_state(dev(U))
+    many = strips.LocalStrips(DG, p, n_strips)
+    many.set_state(dev(U))
+    np.testing.assert_array_equal(many.rhs(0.3).cpu().numpy(), one.rhs(0.3).cpu().numpy())
+    for _ in range(5):
+        dt = one.cfl_dt(0.2)
+        assert many.cfl_dt(0.2) == dt
+        one.step(dt)
+        many.step(dt)
+    a, b = one.get_state().cpu().numpy(), many.get_state().cpu().numpy()
+    assert np.isfinite(a).all()
+    np.testing.assert_array_equal(b, a)
+    assert many.time == one.time
+    if p["q_planet"] > 0:
+        t1, tn = one.torque(one.time), many.torque(one.time)
+        assert abs(t1 - tn) < 1e-12 * max(1.0, abs(t1))
+
+
+def test_split_step_api_errors(DG):
+    from paper_1805_01443_b200 import dg as B
+    p, U = W.vortex(8, 2, rk=2)
+    g = DG(p)
+    g.set_state(dev(U))
+    with pytest.raises(B.DGError):
+        g.substep()                                         # no split step in progress
+    g.step_begin(0.01)
+    with pytest.raises(B.DGError):
+        g.step(0.01)                                        # a split step is in progress
+    g.substep()
+    with pytest.raises(B.DGError):
+        g.step_end()                                        # one sub-step missing
+    g.substep()
+    with pytest.raises(B.DGError):
+        g.substep()                                         # all done
+    g.step_end()
+    g2 = DG(p)
+    g2.set_state(dev(U))
+    g2.step(0.01)
+    np.testing.assert_array_equal(g.get_state().cpu().numpy(), g2.get_state().cpu().numpy())
