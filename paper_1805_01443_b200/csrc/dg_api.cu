@@ -316,6 +316,7 @@ int finish_set_state(dg_ctx* c) {
   }
   c->has_state = true;
   c->wmax_valid = false;
+  c->step_active = false;   // a new state abandons a split step in progress
   c->t = c->p.t0;
   return DG_OK;
 }
