@@ -438,8 +438,12 @@ def step_arrays(p: dict, f_damp: float) -> float:
     rk = p["rk"]
     if rk <= 3:
         arrays, sub = 2 + 3 * (rk - 1), rk
+    elif rk == 4:
+        # Table 1's scheme in its low-storage form (the library's default for rk 4): 2 + 3 + 3, then y_4, u^n -> dt L(y_4),
+        # y_5 (4), then y_5, y_3, y_4, dt L(y_4) -> u^{n+1} (5)
+        arrays, sub = 17, 5
     else:
-        nz = {4: [0, 1, 2, 3, 4], 5: [0, 1, 2, 3, 4, 3]}[rk]     # non-zero a_{i+1,j}, j < i (last row: b)
+        nz = {5: [0, 1, 2, 3, 4, 3]}[rk]     # non-zero a_{i+1,j}, j < i (last row: b)
         sub = len(nz)
         arrays = 0
         for i in range(sub):
@@ -459,7 +463,7 @@ def run_variants(args):
     peak, peak_src = load_peaks()
     n, m = args.n, args.order
     for name, over in (("ssp33 (bench)", {}), ("ssp33 + limiter", {"limiter": 1}),
-                       ("rk4: SSP-RK(5,4), paper Table 1", {"rk": 4}), ("rk5: Cash-Karp, paper Table 2", {"rk": 5}),
+                       ("rk4: SSP-RK(5,4), paper Table 1 (low-storage form)", {"rk": 4}), ("rk5: Cash-Karp, paper Table 2", {"rk": 5}),
                        ("rk5 + limiter", {"rk": 5, "limiter": 1}), ("ssp33, HLL flux (isothermal)", {"flux": 1})):
         p, U = W.disc(n, m, planet=True, noise=1e-4)
         p.update(over)

@@ -166,6 +166,8 @@ long long dg_launch_count(const dg_ctx*);
 #define DG_TUNE_ROWS_PER_CTA 1
 #define DG_TUNE_FUSED_CFL    2
 #define DG_TUNE_GEN_PREFETCH 3   /* Butcher sub-steps: L2 prefetch of u^n / earlier slopes: 0 none, 1 at the start of the row, 2 a row ahead, 3 between the x and y phases of the row (default) */
+#define DG_TUNE_RK4_FORM     4   /* rk 4: 1 = Table 1's scheme in its low-storage (Shu-Osher) form, derived from the
+                                   printed tableau (default); 0 = the Butcher form as printed */
 int dg_set_tuning(dg_ctx*, int key, int value);
 
 /* Average-duration probe: enqueue CUDA events around the stage kernels of the next dg_step calls.

@@ -104,6 +104,8 @@ struct dg_ctx {
   int rows_per_cta;
   int fused_cfl;
   int gen_pf;
+  int rk4_low_storage;        // 1: Table 1's scheme in its Shu-Osher form (default), 0: Butcher form
+  Ssp54 ssp54;
   bool step_active;           // between dg_step_begin and dg_step_end
   int step_next;              // next sub-step of the split step
   double step_dt;
@@ -202,16 +204,18 @@ struct GenArgs {               // K_GEN / K_GENL: out = u^n + sum_j kc[j] kin[j]
   const double* kin[MAXK];
   double kc[MAXK];
   double kself;
+  double kbase = 1.0;
   double* kout;
 };
 
 int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout, double a, double b,
-                 double dt, double t, int kind, const GenArgs* ga = nullptr) {
+                 double dt, double t, int kind, const GenArgs* ga = nullptr, double nfac = -1.0) {
+  // nfac >= 0: the factor of dt N in the output when it is not b (low-storage RK(5,4))
   StageArgs A{};
   const bool gen = kind == K_GEN || kind == K_GENL;
-  const double beta = kind == K_RHS ? 1.0 : (gen ? dt : b * dt);
+  const double beta = kind == K_RHS ? 1.0 : (gen ? dt : (nfac >= 0.0 ? nfac : b) * dt);
   if (gen) {
-    A.nk = ga->nk; A.kself = ga->kself; A.kout = ga->kout; A.gen_pf = c->gen_pf;
+    A.nk = ga->nk; A.kself = ga->kself; A.kbase = ga->kbase; A.kout = ga->kout; A.gen_pf = c->gen_pf;
     for (int k = 0; k < ga->nk; ++k) { A.kin[k] = ga->kin[k]; A.kc[k] = ga->kc[k]; }
   }
   A.qprev = qprev; A.qn = qn; A.qout = qout; A.q0 = c->q0();
@@ -389,7 +393,26 @@ int launch_limit(dg_ctx* c, double* Q, bool final_, double dt) {
 inline int substep_out(int A, int i) { return (A + 1 + (i & 1)) % 3; }
 inline int substep_in(int A, int i) { return i == 0 ? A : substep_out(A, i - 1); }
 
-struct StepPlan { int A, k; bool damp, lim, fuse_tail; double dt; double* stages; };
+struct StepPlan { int A, k; bool damp, lim, fuse_tail, fast4; double dt; double* stages; };
+
+// input and output arrays of sub-step i.  Low-storage RK(5,4): u^n in A, y_2 -> B, y_3 -> C, y_4 -> B,
+// y_5 -> slope buffer 1 (dt L(y_4) sits in slope buffer 0), u^{n+1} -> A (u^n is not read by the last sub-step).
+double* substep_in_ptr(const dg_ctx* c, const StepPlan& P, int i) {
+  if (P.fast4) {
+    const int B = (P.A + 1) % 3, Cc = (P.A + 2) % 3;
+    switch (i) { case 0: return c->q(P.A); case 1: return c->q(B); case 2: return c->q(Cc); case 3: return c->q(B);
+                 default: return c->kbuf(1); }
+  }
+  return c->q(substep_in(P.A, i));
+}
+double* substep_out_ptr(const dg_ctx* c, const StepPlan& P, int i) {
+  if (P.fast4) {
+    const int B = (P.A + 1) % 3, Cc = (P.A + 2) % 3;
+    switch (i) { case 0: return c->q(B); case 1: return c->q(Cc); case 2: return c->q(B); case 3: return c->kbuf(1);
+                 default: return c->q(P.A); }
+  }
+  return c->q(substep_out(P.A, i));
+}
 
 StepPlan make_plan(const dg_ctx* c, double dt, double* stages) {
   StepPlan P{};
@@ -398,6 +421,7 @@ StepPlan make_plan(const dg_ctx* c, double dt, double* stages) {
   P.damp = has_damping(c->p);
   P.lim = c->p.limiter != 0;
   P.fuse_tail = !stages && (c->fused_cfl || P.damp);   // damping + CFL ride on the step's last kernel
+  P.fast4 = c->p.rk == 4 && c->rk4_low_storage && c->ssp54.ok;
   P.dt = dt;
   P.stages = stages;
   return P;
@@ -412,11 +436,42 @@ int step_begin(dg_ctx* c, const StepPlan& P) {
 int run_substep(dg_ctx* c, const StepPlan& P, int i) {
   const double dt = P.dt;
   const bool last = i + 1 == P.k;
-  const double* qin = c->q(substep_in(P.A, i));
+  const double* qin = substep_in_ptr(c, P, i);
   const double* qn = c->q(P.A);
-  double* qout = c->q(substep_out(P.A, i));
+  double* qout = substep_out_ptr(c, P, i);
   int e;
-  if (c->p.rk <= 3) {
+  if (P.fast4) {
+    // Table 1 in its low-storage form (dg_tables.h): three arrays per sub-step for the
+    // first three, instead of all earlier slopes
+    const Ssp54& S = c->ssp54;
+    ButcherTableau bt;
+    butcher_tableau(4, &bt);
+    const double ts = c->t + bt.c[i] * dt;
+    const int B = (P.A + 1) % 3, Cc = (P.A + 2) % 3;
+    if (i == 0) {
+      e = launch_stage(c, qin, qn, qout, 0.0, 1.0, dt, ts, K_FIRST, nullptr, S.beta[0]);
+    } else if (i < 3) {
+      e = launch_stage(c, qin, qn, qout, 1.0 - S.alpha[i], S.alpha[i], dt, ts, K_MID, nullptr, S.beta[i]);
+    } else if (i == 3) {      // y_5, and dt L(y_4) kept for the last sub-step
+      GenArgs ga{};
+      ga.kbase = 1.0 - S.alpha[3];
+      ga.nk = 1; ga.kin[0] = c->q(B); ga.kc[0] = S.alpha[3];
+      ga.kself = S.beta[3];
+      ga.kout = c->kbuf(0);
+      e = launch_stage(c, qin, qn, qout, 0.0, 0.0, dt, ts, K_GEN, &ga);
+    } else {                  // u^{n+1} = c2 y_3 + c3 y_4 + c4 y_5 + d3 dt L(y_4) + d4 dt L(y_5)
+      GenArgs ga{};
+      ga.kbase = S.c4;        // base array: y_5 itself
+      ga.nk = 3;
+      ga.kin[0] = c->q(Cc); ga.kc[0] = S.c2;
+      ga.kin[1] = c->q(B); ga.kc[1] = S.c3;
+      ga.kin[2] = c->kbuf(0); ga.kc[2] = S.d3;
+      ga.kself = S.d4;
+      ga.kout = nullptr;
+      const int kind = (P.fuse_tail && !P.lim) ? K_GENL : K_GEN;
+      e = launch_stage(c, qin, qin, qout, 0.0, 0.0, dt, ts, kind, &ga);
+    }
+  } else if (c->p.rk <= 3) {
     // SSP-RK in Shu-Osher form, stage times c = (0,1) / (0,1,1/2)
     const int last_kind = (P.fuse_tail && !P.lim) ? (P.damp ? K_LASTD : K_LAST) : K_MID;
     if (i == 0)                  e = launch_stage(c, qin, qn, qout, 0.0, 1.0, dt, c->t, K_FIRST);
@@ -448,7 +503,7 @@ int run_substep(dg_ctx* c, const StepPlan& P, int i) {
 }
 
 int step_end(dg_ctx* c, const StepPlan& P) {
-  c->cur = substep_out(P.A, P.k - 1);
+  c->cur = P.fast4 ? P.A : substep_out(P.A, P.k - 1);
   c->wmax_valid = P.fuse_tail && c->fused_cfl;
   if (!P.fuse_tail && P.damp) {   // damping as its own pass (debug path, or nothing to ride on)
     int e = launch_damp(c, c->q(c->cur), P.dt);
@@ -512,6 +567,12 @@ int dg_init(const dg_params* p, void* workspace, size_t ws_bytes, void* cuda_str
     c->rows_per_cta = (int)std::max(4L, std::min(16L, rows));
   }
   c->fused_cfl = 1;
+  c->rk4_low_storage = 1;
+  {
+    ButcherTableau bt;
+    butcher_tableau(4, &bt);
+    c->ssp54 = ssp54_from_butcher(bt);
+  }
   c->step_active = false;
   c->step_next = 0;
   c->gen_pf = 3;
@@ -700,10 +761,15 @@ int dg_halo_layout(dg_ctx* c, size_t offsets[4], size_t* row_bytes) {
   if (!c || !offsets || !row_bytes) return c ? fail(c, DG_EINVAL, "dg_halo_layout: null") : DG_EINVAL;
   if (!c->has_state) return fail(c, DG_ESTATE, "dg_halo_layout: state not set");
   // the array the next stage kernel reads: the sub-step's input inside a split step, else the current state
-  const int buf = c->step_active ? substep_in(c->step_A, c->step_next) : c->cur;
+  size_t off = c->L.off_q[c->cur];
+  if (c->step_active) {
+    StepPlan P = make_plan(c, c->step_dt, nullptr);
+    P.A = c->step_A;
+    off = (size_t)(reinterpret_cast<char*>(substep_in_ptr(c, P, c->step_next)) - c->ws);
+  }
   *row_bytes = c->L.row_bytes;
-  offsets[0] = c->L.off_q[buf];                                                 // first row: the south neighbour's north halo
-  offsets[1] = c->L.off_q[buf] + (size_t)(c->p.ny - 1) * c->L.row_bytes;          // last row: the north neighbour's south halo
+  offsets[0] = off;                                                  // first row: the south neighbour's north halo
+  offsets[1] = off + (size_t)(c->p.ny - 1) * c->L.row_bytes;          // last row: the north neighbour's south halo
   offsets[2] = c->p.halo_south ? c->L.off_haloS : (size_t)-1;
   offsets[3] = c->p.halo_north ? c->L.off_haloN : (size_t)-1;
   return DG_OK;
@@ -743,6 +809,10 @@ int dg_set_tuning(dg_ctx* c, int key, int value) {
     case DG_TUNE_FUSED_CFL:
       c->fused_cfl = value ? 1 : 0;
       c->wmax_valid = false;
+      return DG_OK;
+    case DG_TUNE_RK4_FORM:
+      if (c->step_active) return fail(c, DG_ESTATE, "a split step is in progress");
+      c->rk4_low_storage = value ? 1 : 0;
       return DG_OK;
     case DG_TUNE_GEN_PREFETCH:
       if (value < 0 || value > 3) return fail(c, DG_EINVAL, "prefetch mode must be 0..3");

@@ -32,7 +32,7 @@ enum : int {          // KIND: what the epilogue of the stage does
   K_LAST  = 3,        // K_MID + fused CFL wave-speed reduction
   K_LASTD = 4,        // K_LAST + wave-killing relaxation
   K_GEN   = 5,        // Butcher-form sub-step: K_i = dt N(y_i) -> kout,
-                      //   out = u^n + sum_j kc[j] kin[j] + kself K_i
+                      //   out = kbase u^n + sum_j kc[j] kin[j] + kself K_i
   K_GENL  = 6,        // K_GEN of the last sub-step: no kout, fused CFL reduction, wave-killing if enabled
   K_COUNT = 7,
 };
@@ -109,6 +109,7 @@ struct StageArgs {
   const double* kin[MAXK];
   double kc[MAXK];
   double kself;
+  double kbase;               // coefficient of the base array qn (1 in the Butcher form)
   double* kout;
   int nk;
   int gen_pf;                 // L2 prefetch of the epilogue's inputs: 0 none, 1 row start, 2 a row ahead (evicted before use: 1.7x DRAM reads), 3 at the x/y phase boundary
@@ -764,7 +765,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           if (gen) {                               // out is K_i = dt N(y_i) here
             const double K = out;
             if (KIND == K_GEN && A.kout && valid) A.kout[cell_off + e] = K;
-            out = gb[rr];
+            out = A.kbase * gb[rr];
 #pragma unroll
             for (int k = 0; k < MAXK; ++k) out = fma(A.kc[k], gk[k][rr], out);   // kc = 0 beyond nk
             out = fma(A.kself, K, out);

@@ -179,4 +179,37 @@ inline bool butcher_tableau(int rk, ButcherTableau* B) {
   return false;
 }
 
+// Table 1's scheme in the low-storage (Shu-Osher) form it has by construction: rows 2..5 of the printed
+// tableau are multiples of the row above plus one new entry, a_{i+1,j} = alpha_i a_{ij} (j < i), so that
+//   y_{i+1} = (1 - alpha_i) u^n + alpha_i y_i + beta_i dt L(y_i),  i = 1..4  (alpha_1 = 1),
+//   u^{n+1} = c2 y_3 + c3 y_4 + c4 y_5 + d3 dt L(y_4) + d4 dt L(y_5),
+// all coefficients solved from the printed a, b (b renormalised).  Algebraically the Butcher form; in
+// floating point it differs from it at the printed tableau's own precision (1e-14).  `ok` is false if the
+// tableau does not have that structure to 1e-12 (then the Butcher form is used).
+struct Ssp54 { bool ok; double alpha[4], beta[4], c2, c3, c4, d3, d4; };
+
+inline Ssp54 ssp54_from_butcher(const ButcherTableau& B) {
+  Ssp54 S{};
+  S.ok = B.s == 5;
+  if (!S.ok) return S;
+  S.alpha[0] = 1.0;
+  S.beta[0] = B.a[1][0];
+  for (int i = 1; i < 4; ++i) {
+    S.alpha[i] = B.a[i + 1][0] / B.a[i][0];
+    S.beta[i] = B.a[i + 1][i];
+    for (int j = 0; j < i; ++j)
+      if (std::fabs(B.a[i + 1][j] - S.alpha[i] * B.a[i][j]) > 1e-12) S.ok = false;
+  }
+  const double r = B.b[2] / B.a[3][2];                       // c3 + alpha_4 c4
+  S.c2 = B.b[0] / B.a[2][0] - S.alpha[2] * r;
+  const double sum = 1.0 - S.c2;                              // c3 + c4
+  S.c4 = (sum - r) / (1.0 - S.alpha[3]);
+  S.c3 = sum - S.c4;
+  S.d3 = B.b[3] - S.c4 * B.a[4][3];
+  S.d4 = B.b[4];
+  const double b1 = S.c2 * B.a[2][1] + S.c3 * B.a[3][1] + S.c4 * B.a[4][1];
+  if (std::fabs(b1 - B.b[1]) > 1e-12 || !(S.c2 > 0 && S.c3 > 0 && S.c4 > 0 && S.d3 > 0)) S.ok = false;
+  return S;
+}
+
 }  // namespace dg

@@ -563,7 +563,8 @@ def test_literal_baseline_disc_runs_with_the_limiter(DG):
 
 # ------------------------------------------------------------------------------------------------
 # NEXT-4: strips of a domain decomposed along y, halo rows exchanged before every sub-step
-@pytest.mark.parametrize("name,n_strips", [("vortex", 2), ("vortex", 3), ("disc", 4), ("disc_rk5_lim", 3), ("hllc", 2)])
+@pytest.mark.parametrize("name,n_strips", [("vortex", 2), ("vortex", 3), ("disc", 4), ("disc_rk5_lim", 3), ("hllc", 2),
+                                           ("disc_rk4", 2)])
 def test_strip_decomposition_reproduces_the_undivided_domain(DG, name, n_strips):
     """All strips on one GPU (`strips.LocalStrips`): the stage kernels read the neighbour strip's boundary rows
     from their halo rows.  Grids and boxes with binary-exact spacings, so the strips' node coordinates are the
@@ -574,6 +575,8 @@ def test_strip_decomposition_reproduces_the_undivided_domain(DG, name, n_strips)
         p.update(x1=8.0, y1=8.0)                           # dx = 1/4: exact
     elif name == "disc":
         p, U = W.disc(64, 4, planet=True, noise=1e-4, half_width=2.0)
+    elif name == "disc_rk4":
+        p, U = W.disc(64, 5, planet=True, noise=1e-4, half_width=2.0, rk=4)
     elif name == "disc_rk5_lim":
         p, U = W.disc(64, 3, planet=True, noise=1e-4, half_width=2.0, rk=5)
         p.update(limiter=1, damp_in_r0=0.5, damp_in_r1=0.4)
@@ -620,3 +623,28 @@ def test_split_step_api_errors(DG):
     g2.set_state(dev(U))
     g2.step(0.01)
     np.testing.assert_array_equal(g.get_state().cpu().numpy(), g2.get_state().cpu().numpy())
+
+
+def test_rk4_low_storage_form_equals_the_butcher_form(DG):
+    """rk 4 runs Table 1's scheme in the low-storage form derived from the printed tableau
+    (DG_TUNE_RK4_FORM = 1, default); the Butcher form as printed (= 0) and the oracle give the same step to 1e-12,
+    with and without the limiter / wave-killing tail."""
+    for lim in (0, 1):
+        p, U = W.disc(48, 4, planet=True, noise=1e-4, rk=4)
+        p["limiter"] = lim
+        ref = oracle.RefDG(p, omp=True)
+        ref.set_state(U)
+        dt = ref.cfl_dt(0.2)
+        ref.step(dt)
+        ref.step(dt)
+        outs = []
+        for form in (1, 0):
+            g = DG(p)
+            g.set_tuning(4, form)
+            g.set_state(dev(U))
+            g.step(dt)
+            g.step(dt)
+            outs.append(g.get_state().cpu().numpy())
+            assert rel_err(outs[-1], ref.get_state()) < TOL_STAGE
+            assert abs(g.cfl_dt(0.2) / ref.cfl_dt(0.2) - 1.0) < 1e-12
+        assert rel_err(outs[0], outs[1]) < TOL_STAGE
