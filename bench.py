@@ -439,9 +439,9 @@ def step_arrays(p: dict, f_damp: float) -> float:
     if rk <= 3:
         arrays, sub = 2 + 3 * (rk - 1), rk
     elif rk == 4:
-        # Table 1's scheme in its low-storage form (the library's default for rk 4): 2 + 3 + 3, then y_4, u^n -> dt L(y_4),
-        # y_5 (4), then y_5, y_3, y_4, dt L(y_4) -> u^{n+1} (5)
-        arrays, sub = 17, 5
+        # Table 1's scheme in its low-storage form (the library's default for rk 4): 2 + 3 + 3 + 3, then
+        # y_5, y_3, y_4, u^n -> u^{n+1} (5)
+        arrays, sub = 16, 5
     else:
         nz = {5: [0, 1, 2, 3, 4, 3]}[rk]     # non-zero a_{i+1,j}, j < i (last row: b)
         sub = len(nz)

@@ -396,7 +396,7 @@ inline int substep_in(int A, int i) { return i == 0 ? A : substep_out(A, i - 1);
 struct StepPlan { int A, k; bool damp, lim, fuse_tail, fast4; double dt; double* stages; };
 
 // input and output arrays of sub-step i.  Low-storage RK(5,4): u^n in A, y_2 -> B, y_3 -> C, y_4 -> B,
-// y_5 -> slope buffer 1 (dt L(y_4) sits in slope buffer 0), u^{n+1} -> A (u^n is not read by the last sub-step).
+// y_5 -> spare buffer 1, u^{n+1} -> spare buffer 0, which then trades places with A (step_end).
 double* substep_in_ptr(const dg_ctx* c, const StepPlan& P, int i) {
   if (P.fast4) {
     const int B = (P.A + 1) % 3, Cc = (P.A + 2) % 3;
@@ -409,7 +409,7 @@ double* substep_out_ptr(const dg_ctx* c, const StepPlan& P, int i) {
   if (P.fast4) {
     const int B = (P.A + 1) % 3, Cc = (P.A + 2) % 3;
     switch (i) { case 0: return c->q(B); case 1: return c->q(Cc); case 2: return c->q(B); case 3: return c->kbuf(1);
-                 default: return c->q(P.A); }
+                 default: return c->kbuf(0); }
   }
   return c->q(substep_out(P.A, i));
 }
@@ -452,20 +452,18 @@ int run_substep(dg_ctx* c, const StepPlan& P, int i) {
       e = launch_stage(c, qin, qn, qout, 0.0, 1.0, dt, ts, K_FIRST, nullptr, S.beta[0]);
     } else if (i < 3) {
       e = launch_stage(c, qin, qn, qout, 1.0 - S.alpha[i], S.alpha[i], dt, ts, K_MID, nullptr, S.beta[i]);
-    } else if (i == 3) {      // y_5, and dt L(y_4) kept for the last sub-step
+    } else if (i == 3) {
+      e = launch_stage(c, qin, qn, qout, 1.0 - S.alpha[3], S.alpha[3], dt, ts, K_MID, nullptr, S.beta[3]);
+    } else {
+      // u^{n+1} = c2 y_3 + c3 y_4 + c4 y_5 + d3 dt L(y_4) + d4 dt L(y_5), with dt L(y_4) eliminated through
+      // y_5 = (1 - alpha_4) u^n + alpha_4 y_4 + beta_4 dt L(y_4): no slope is ever stored
+      const double r = S.d3 / S.beta[3];
       GenArgs ga{};
-      ga.kbase = 1.0 - S.alpha[3];
-      ga.nk = 1; ga.kin[0] = c->q(B); ga.kc[0] = S.alpha[3];
-      ga.kself = S.beta[3];
-      ga.kout = c->kbuf(0);
-      e = launch_stage(c, qin, qn, qout, 0.0, 0.0, dt, ts, K_GEN, &ga);
-    } else {                  // u^{n+1} = c2 y_3 + c3 y_4 + c4 y_5 + d3 dt L(y_4) + d4 dt L(y_5)
-      GenArgs ga{};
-      ga.kbase = S.c4;        // base array: y_5 itself
+      ga.kbase = S.c4 + r;    // base array: y_5 itself
       ga.nk = 3;
       ga.kin[0] = c->q(Cc); ga.kc[0] = S.c2;
-      ga.kin[1] = c->q(B); ga.kc[1] = S.c3;
-      ga.kin[2] = c->kbuf(0); ga.kc[2] = S.d3;
+      ga.kin[1] = c->q(B); ga.kc[1] = S.c3 - r * S.alpha[3];
+      ga.kin[2] = c->q(P.A); ga.kc[2] = -r * (1.0 - S.alpha[3]);
       ga.kself = S.d4;
       ga.kout = nullptr;
       const int kind = (P.fuse_tail && !P.lim) ? K_GENL : K_GEN;
@@ -503,7 +501,12 @@ int run_substep(dg_ctx* c, const StepPlan& P, int i) {
 }
 
 int step_end(dg_ctx* c, const StepPlan& P) {
-  c->cur = P.fast4 ? P.A : substep_out(P.A, P.k - 1);
+  if (P.fast4) {            // the new state sits in spare buffer 0: it becomes buffer A, the old u^n the spare
+    std::swap(c->L.off_q[P.A], c->L.off_k[0]);
+    c->cur = P.A;
+  } else {
+    c->cur = substep_out(P.A, P.k - 1);
+  }
   c->wmax_valid = P.fuse_tail && c->fused_cfl;
   if (!P.fuse_tail && P.damp) {   // damping as its own pass (debug path, or nothing to ride on)
     int e = launch_damp(c, c->q(c->cur), P.dt);

@@ -182,7 +182,7 @@ inline bool butcher_tableau(int rk, ButcherTableau* B) {
 // Table 1's scheme in the low-storage (Shu-Osher) form it has by construction: rows 2..5 of the printed
 // tableau are multiples of the row above plus one new entry, a_{i+1,j} = alpha_i a_{ij} (j < i), so that
 //   y_{i+1} = (1 - alpha_i) u^n + alpha_i y_i + beta_i dt L(y_i),  i = 1..4  (alpha_1 = 1),
-//   u^{n+1} = c2 y_3 + c3 y_4 + c4 y_5 + d3 dt L(y_4) + d4 dt L(y_5),
+//   u^{n+1} = c2 y_3 + c3 y_4 + c4 y_5 + d3 dt L(y_4) + d4 dt L(y_5)   (dt L(y_4) = (y_5 - (1-alpha_4) u^n - alpha_4 y_4)/beta_4),
 // all coefficients solved from the printed a, b (b renormalised).  Algebraically the Butcher form; in
 // floating point it differs from it at the printed tableau's own precision (1e-14).  `ok` is false if the
 // tableau does not have that structure to 1e-12 (then the Butcher form is used).
