@@ -45,8 +45,9 @@ typedef struct {
   int32_t order;                  /* m = 1..5: m x m modes per cell and variable */
   int32_t rk;                     /* 2: SSP-RK(2,2), 3: SSP-RK(3,3) (Gottlieb & Shu 1998);
                                      4: the five-stage fourth-order SSP scheme of Table 1,
-                                     5: the six-stage Cash-Karp scheme of Table 2, both in
-                                     Butcher form (Appendix A); see dg_rk_stages */
+                                     5: the six-stage Cash-Karp scheme of Table 2, both printed in
+                                     Butcher form (Appendix A); rk 4 is evaluated in the equivalent
+                                     low-storage form solved from the printed tableau (DG_TUNE_RK4_FORM); see dg_rk_stages */
   int32_t bc;                     /* 0 periodic; 1 transmissive (exterior trace = interior);
                                      2 frozen: exterior trace = trace of the state given to the last
                                      dg_set_state*, same boundary cell, same face point */
