@@ -264,6 +264,14 @@ __device__ __forceinline__ void column_trace(const double* cell, int stride, int
   }
 }
 
+// A read-only global load the compiler may not move: issued where it is written (a prefetch into registers
+// for a later row), not sunk to its first use.
+__device__ __forceinline__ double ldg_here(const double* p) {
+  double v;
+  asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+  return v;
+}
+
 __device__ __forceinline__ double shfl_up1(double x) { return __shfl_up_sync(FULL, x, 1); }
 __device__ __forceinline__ double shfl_dn1(double x) { return __shfl_down_sync(FULL, x, 1); }
 __device__ __forceinline__ Wave<0> shfl_dn1(const Wave<0>& w) { return Wave<0>{shfl_dn1(w.lam)}; }
@@ -523,7 +531,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     double enext[M];                             // next row's edge lines: in flight during this whole row
 #pragma unroll
     for (int q = 0; q < M; ++q)
-      enext[q] = (edge_src && more) ? __ldg(edge_src + (size_t)(j + 1) * row_stride + q * 32) : 0.0;
+      enext[q] = (edge_src && more) ? ldg_here(edge_src + (size_t)(j + 1) * row_stride + q * 32) : 0.0;
     {
       const int r = w;
       tile_wait(t);
