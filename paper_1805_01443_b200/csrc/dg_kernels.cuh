@@ -16,6 +16,14 @@
 //   Y phase  warp q owns the xi-column q: the same along y with G, plus the gravity source, plus the
 //            S/N faces (row below carried in registers while marching, row above read ahead), then
 //            the RK combine (and damping) and the store of u^(s).
+// Compile-time variants: EOS (ideal gas / locally isothermal), GRAV (none / star / star + planet), KIND (what
+// the epilogue does: rhs only, SSP stages, Butcher-form sub-steps of SURVEY.md 8(f) NEXT-2), FLUX (local
+// Lax-Friedrichs / HLLC-HLL, NEXT-4).  At a halo edge of a strip decomposition the out-of-strip row is
+// fetched from a halo row like any other tile (StageArgs::haloS / haloN).
+//
+// Why 2 thread blocks of 5 warps per SM at M = 5: 4 tile-sized buffers of 25.6 KB + tables = 114 KB of shared
+// memory per block, and 168 registers is the most that lets 10 warps reside (registers are handed out to
+// warps in groups of four: 12 x 168 x 32 <= 64 Ki).
 #pragma once
 #include <cstdint>
 
