@@ -346,8 +346,18 @@ constexpr size_t stage_smem_bytes() {
   return ((size_t)(NST + 1) * 4 * M * M * 32 + (size_t)M * M * 32 + (size_t)4 * M * 32) * sizeof(double) + 64;
 }
 
+// Warps per thread block: M workers, plus -- at M = 5, in the stages that carry the fused CFL reduction -- one helper
+// warp that issues the TMA copies / prefetches and does that reduction.  It costs no occupancy there (registers are
+// allocated to warps in groups of four, so 2 x 6 warps of 168 registers fit exactly like 2 x 5) and takes ~150
+// instructions per row off worker warp 0's critical path: last stage 0.645 ms instead of 0.670 at 1024^2.  In the
+// stages without the reduction the extra warp only costs (+2 % measured), so they keep M warps.
+template <int M, int KIND> struct StageWarps {
+  static constexpr int helper = (M == 5 && (KIND == K_LAST || KIND == K_LASTD || KIND == K_GENL)) ? 1 : 0;
+  static constexpr int threads = (M + helper) * 32;
+};
+
 template <int M, int EOS, int GRAV, int KIND, int MINB, int FLUX = 0>
-__global__ void __launch_bounds__(M * 32, MINB)
+__global__ void __launch_bounds__((StageWarps<M, KIND>::threads), MINB)
 stage_kernel(const __grid_constant__ StageArgs A) {
   constexpr bool grav = GRAV != G_NONE;
   constexpr bool need_ri = EOS == 1 || grav;
@@ -369,6 +379,10 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   const int tid = threadIdx.x;
   const int lane = tid & 31;
   const int w = tid >> 5;                        // eta-line (X phase) / xi-column (Y phase)
+  constexpr bool HELPER = StageWarps<M, KIND>::helper != 0;
+  constexpr int ISSUER = HELPER ? M * 32 : 0;    // the thread that issues copies and prefetches
+  constexpr int CFLW = HELPER ? M : 0;           // the warp that does the fused CFL reduction
+  const bool worker = w < M;
   const int ib = blockIdx.x;
   const int i = ib * 32 + lane;
   const Geom& g = A.g;
@@ -381,7 +395,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 
   const double xc = g.x0 + (i + 0.5) * g.dx;
   const double xW = g.x0 + i * g.dx, xE = g.x0 + (i + 1) * g.dx;
-  const double xq_col = xc + g.hdx * T.xi[w];    // x of this thread's column (Y phase)
+  const double xq_col = xc + g.hdx * T.xi[worker ? w : 0];    // x of this thread's column (Y phase)
 
   // x-neighbour cells outside this block: (cell index, or -1 when there is none).  Lanes 0..7 of
   // warp r fetch line r of those two cells straight from L2 (their own blocks are loading the same
@@ -390,7 +404,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   const int iRn = ib * 32 + 32 < g.nx ? ib * 32 + 32 : (g.bc == 0 ? 0 : -1);
   const bool haveL = iLn >= 0, haveR = iRn >= 0;
   const double* edge_src = nullptr;
-  if (lane < 8) {
+  if (lane < 8 && worker) {
     const int ic = lane < 4 ? iLn : iRn;
     if (ic >= 0) edge_src = A.qprev + (size_t)(ic >> 5) * BS + (ic & 31) + (size_t)(((lane & 3) * M + w) * M) * 32;
   }
@@ -444,13 +458,13 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     for (int k = 0; k < A.nk; ++k) bulk_prefetch_l2(A.kin[k] + off, TILE_BYTES);
   };
 
-  if (tid == 0) {
+  if (tid == ISSUER) {
 #pragma unroll
     for (int s = 0; s <= NST; ++s) mbar_init(mbar + s, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  if (tid == 0) {
+  if (tid == ISSUER) {
     tile_issue(0);
     tile_issue(1);
     tile_issue(2);
@@ -467,8 +481,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   // numerical flux (x2) through the south face of the segment's first row, column q = w: the only
   // face whose two sides are both evaluated here; afterwards a row's N flux is the next row's S flux
   double HS[4];
-  double spmax = 0.0;                            // running CFL wave-speed maximum of this lane (warp 0)
-  {
+  double spmax = 0.0;                            // running CFL wave-speed maximum of this lane (warp CFLW)
+  if (worker) {
     const double yS = g.y0 + j0 * g.dy;
     double cs2 = 0.0, ciso = 0.0;
     if (EOS == 1) {
@@ -500,7 +514,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   for (int j = j0; j < j1; ++j) {
     const int t = j - j0 + 1;                    // tile index of row j
     const bool more = j + 1 < j1;
-    if (tid == 0) {
+    if (tid == ISSUER) {
       fence_proxy_async();                       // the slots about to be refilled were read through the generic proxy
       if (more) tile_issue(t + 2);               // row j+2 -> the slot row j-1 has just left
       if (use_un && j > j0) un_issue(j);         // sN is free again
@@ -512,7 +526,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     const double yc = g.y0 + (j + 0.5) * g.dy;
 
     // fused CFL wave speed of the row finished in the previous iteration (row a10)
-    if (do_cfl && w == 0 && j > j0) {
+    if (do_cfl && w == CFLW && j > j0) {
       double avg[4];
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
@@ -540,7 +554,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 #pragma unroll
     for (int q = 0; q < M; ++q)
       enext[q] = (edge_src && more) ? ldg_here(edge_src + (size_t)(j + 1) * row_stride + q * 32) : 0.0;
-    {
+    if (worker) {
       const int r = w;
       tile_wait(t);
       const double yr = yc + g.hdy * T.xi[r];
@@ -657,9 +671,9 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     }
     __syncthreads();
 
-    if (gen && A.gen_pf == 3 && tid == 32 % (M * 32)) prefetch_gen(j);
+    if (gen && A.gen_pf == 3 && tid == (HELPER ? ISSUER : 32 % (M * 32))) prefetch_gen(j);
     // =========================== Y phase: xi-column q = w ===========================
-    {
+    if (worker) {
       const int q = w;
       const double xq = xq_col;
       double acc[4][M];
@@ -800,7 +814,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     __syncthreads();
   }
   // CFL wave speed of the last row of the segment, then one reduction per thread block
-  if (do_cfl && w == 0) {
+  if (do_cfl && w == CFLW) {
     double avg[4];
 #pragma unroll
     for (int v = 0; v < 4; ++v) {

@@ -27,7 +27,7 @@ cudaError_t launch_stage_variant(const StageArgs& A, dim3 grid, cudaStream_t str
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  kern<<<grid, M * 32, smem, stream>>>(A);
+  kern<<<grid, StageWarps<M, KIND>::threads, smem, stream>>>(A);
   return cudaGetLastError();
 }
 
