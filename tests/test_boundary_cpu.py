@@ -107,11 +107,11 @@ def test_product_never_imports_oracle():
 
 def test_sass_uses_bulk_async_copy():
     """The stage kernel's tile ring is fed by TMA bulk copies (UBLKCP in SASS) and waits on mbarriers."""
-    from paper_1805_01443_b200.build import LIB, build
+    from paper_1805_01443_b200.build import LIB, OBJ_DIR, build
     build()
-    out = subprocess.run(["cuobjdump", "-sass", "-fun", "stage_kernel", LIB], capture_output=True, text=True)
-    if out.returncode != 0 or "UBLKCP" not in out.stdout:
-        out = subprocess.run(["cuobjdump", "-sass", LIB], capture_output=True, text=True)
+    obj = os.path.join(OBJ_DIR, "dg_stage_m2.o")          # one small translation unit is enough (and quick)
+    target = obj if os.path.exists(obj) else LIB
+    out = subprocess.run(["cuobjdump", "-sass", target], capture_output=True, text=True)
     assert "UBLKCP" in out.stdout
     assert "SYNCS" in out.stdout          # mbarrier arrive / try_wait
 
