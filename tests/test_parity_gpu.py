@@ -665,3 +665,33 @@ def test_host_entry_points_next_rows(DG, rk, lim):
     for _ in range(4):
         g2.step(g2.cfl_dt(0.2))
     np.testing.assert_array_equal(hout.numpy(), g2.get_state().cpu().numpy())
+
+
+def test_dist_strip_single_rank_nccl(DG):
+    """`strips.DistStrip` through torch.distributed with the NCCL backend at world_size 1 (the most one GPU
+    allows): the all_reduce plumbing for dt and the torque runs on device tensors, the strip is the whole domain."""
+    import socket
+    import torch.distributed as dist
+    from paper_1805_01443_b200 import strips
+    if dist.is_initialized():
+        pytest.skip("a process group already exists in this process")
+    s_ = socket.socket()
+    s_.bind(("127.0.0.1", 0))
+    port = s_.getsockname()[1]
+    s_.close()
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1)
+    try:
+        p, U = W.disc(64, 3, planet=True, noise=1e-4)
+        s = strips.DistStrip(DG, p)
+        s.set_state(dev(U[s.j0:s.j1]))
+        g = DG(p)
+        g.set_state(dev(U))
+        for _ in range(3):
+            dt = s.cfl_dt(0.2)
+            assert dt == g.cfl_dt(0.2)
+            s.step(dt)
+            g.step(dt)
+        assert torch.equal(s.g.get_state(), g.get_state())
+        assert s.torque(g.time) == g.torque(g.time)
+    finally:
+        dist.destroy_process_group()
