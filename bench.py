@@ -432,22 +432,24 @@ def run_sweep(args):
 
 def step_arrays(p: dict, f_damp: float) -> float:
     """Algorithmic state-sized arrays one time step moves (reads + writes), for any scheme / limiter:
-    SSP forms: 2 + 3 (rk-1); Butcher form sub-step i (0-based, s sub-steps): reads y_i, u^n (one array when
-    i = 0) and the earlier slopes with non-zero coefficient, writes K_i (not the last) and y_{i+1};
-    limiter: one more read per sub-step (writes only the cells it changes); wave-killing: f_damp."""
+    SSP forms: 2 + 3 (rk-1); general schemes: see below; limiter: one more read per sub-step (writes only the
+    cells it changes); wave-killing: f_damp."""
     rk = p["rk"]
+    lim = bool(p.get("limiter"))
     if rk <= 3:
         arrays, sub = 2 + 3 * (rk - 1), rk
-    elif rk == 4:
-        # Table 1's scheme in its low-storage form (the library's default for rk 4): 2 + 3 + 3 + 3, then
-        # y_5, y_3, y_4, u^n -> u^{n+1} (5)
-        arrays, sub = 16, 5
+    elif not lim:
+        # state form (dg_tables.h): sub-step i reads its input, u^n and the earlier states with a non-zero
+        # coefficient, writes one array.  rk 4 (Table 1, low-storage): 2 + 3 + 3 + 3 + 5; rk 5 (Cash-Karp): 2 + 3 + ... + 7
+        arrays, sub = (16, 5) if rk == 4 else (27, 6)
     else:
-        nz = {5: [0, 1, 2, 3, 4, 3]}[rk]     # non-zero a_{i+1,j}, j < i (last row: b)
+        # with the limiter the sub-steps keep Z_i (their result before the earlier slopes' terms) as well:
+        # input, u^n, the earlier Z_j with non-zero coefficient, two arrays written (one in the last sub-step)
+        nz = {4: [0, 1, 2, 3, 4], 5: [0, 1, 2, 3, 4, 3]}[rk]
         sub = len(nz)
         arrays = 0
         for i in range(sub):
-            arrays += (1 if i == 0 else 2) + nz[i] + (1 if i + 1 < sub else 0) + 1
+            arrays += (1 if i == 0 else 2) + nz[i] + (2 if i + 1 < sub else 1)
     if p.get("limiter"):
         arrays += sub
     return arrays + f_damp

@@ -46,8 +46,9 @@ typedef struct {
   int32_t rk;                     /* 2: SSP-RK(2,2), 3: SSP-RK(3,3) (Gottlieb & Shu 1998);
                                      4: the five-stage fourth-order SSP scheme of Table 1,
                                      5: the six-stage Cash-Karp scheme of Table 2, both printed in
-                                     Butcher form (Appendix A); rk 4 is evaluated in the equivalent
-                                     low-storage form solved from the printed tableau (DG_TUNE_RK4_FORM); see dg_rk_stages */
+                                     Butcher form (Appendix A) and evaluated on the stage states
+                                     (coefficients solved from the printed tableau; with the limiter on, in a form that
+                                     keeps the slopes of the limited states); see dg_rk_stages */
   int32_t bc;                     /* 0 periodic; 1 transmissive (exterior trace = interior);
                                      2 frozen: exterior trace = trace of the state given to the last
                                      dg_set_state*, same boundary cell, same face point */
@@ -166,9 +167,9 @@ long long dg_launch_count(const dg_ctx*);
  *   DG_TUNE_FUSED_CFL    : 1 = the last RK stage also reduces the CFL wave speed (default), 0 = separate kernel */
 #define DG_TUNE_ROWS_PER_CTA 1
 #define DG_TUNE_FUSED_CFL    2
-#define DG_TUNE_GEN_PREFETCH 3   /* Butcher sub-steps: L2 prefetch of u^n / earlier slopes: 0 none, 1 at the start of the row, 2 a row ahead, 3 between the x and y phases of the row (default) */
-#define DG_TUNE_RK4_FORM     4   /* rk 4: 1 = Table 1's scheme in its low-storage (Shu-Osher) form, derived from the
-                                   printed tableau (default); 0 = the Butcher form as printed */
+#define DG_TUNE_GEN_PREFETCH 3   /* general sub-steps: L2 prefetch of the earlier stage states: 0 none, 1 at the start of the row, 2 a row ahead, 3 between the x and y phases of the row (default) */
+#define DG_TUNE_RK4_FORM     4   /* rk 4, limiter off: 1 = Table 1's scheme in its low-storage (Shu-Osher) form, from the
+                                   printed tableau's row ratios (default); 0 = the generic state form */
 int dg_set_tuning(dg_ctx*, int key, int value);
 
 /* Average-duration probe: enqueue CUDA events around the stage kernels of the next dg_step calls.

@@ -199,13 +199,11 @@ DampArgs make_damp(const dg_ctx* c, double dt, bool enable = true) {
 // dg_kernels.cuh; K_RHS writes L itself).  The kernel computes a*qn + b*qprev + beta*L with
 // beta = b*dt folded into the derivative / lifting tables and the gravity constants here; the
 // lifting vectors also carry the 1/2 of the Lax-Friedrichs average (the kernel forms 2 x flux).
-struct GenArgs {               // K_GEN / K_GENL: out = u^n + sum_j kc[j] kin[j] + kself K_i, K_i = dt N -> kout
+struct GenArgs {               // K_GEN / K_GENL: out = a u^n + b u + sum_j kc[j] kin[j] + nfac dt N
   int nk;
   const double* kin[MAXK];
   double kc[MAXK];
-  double kself;
-  double kbase = 1.0;
-  double* kout;
+  double* zout = nullptr;
 };
 
 int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout, double a, double b,
@@ -213,9 +211,9 @@ int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout,
   // nfac >= 0: the factor of dt N in the output when it is not b (low-storage RK(5,4))
   StageArgs A{};
   const bool gen = kind == K_GEN || kind == K_GENL;
-  const double beta = kind == K_RHS ? 1.0 : (gen ? dt : (nfac >= 0.0 ? nfac : b) * dt);
+  const double beta = kind == K_RHS ? 1.0 : (nfac >= 0.0 ? nfac : b) * dt;
   if (gen) {
-    A.nk = ga->nk; A.kself = ga->kself; A.kbase = ga->kbase; A.kout = ga->kout; A.gen_pf = c->gen_pf;
+    A.nk = ga->nk; A.zout = ga->zout; A.gen_pf = c->gen_pf;
     for (int k = 0; k < ga->nk; ++k) { A.kin[k] = ga->kin[k]; A.kc[k] = ga->kc[k]; }
   }
   A.qprev = qprev; A.qn = qn; A.qout = qout; A.q0 = c->q0();
@@ -403,6 +401,7 @@ double* substep_in_ptr(const dg_ctx* c, const StepPlan& P, int i) {
     switch (i) { case 0: return c->q(P.A); case 1: return c->q(B); case 2: return c->q(Cc); case 3: return c->q(B);
                  default: return c->kbuf(1); }
   }
+  if (c->p.rk >= 4 && !P.lim) return i == 0 ? c->q(P.A) : c->kbuf(i - 1);     // state form: y_{i+1} in spare buffer i-1
   return c->q(substep_in(P.A, i));
 }
 double* substep_out_ptr(const dg_ctx* c, const StepPlan& P, int i) {
@@ -411,6 +410,7 @@ double* substep_out_ptr(const dg_ctx* c, const StepPlan& P, int i) {
     switch (i) { case 0: return c->q(B); case 1: return c->q(Cc); case 2: return c->q(B); case 3: return c->kbuf(1);
                  default: return c->kbuf(0); }
   }
+  if (c->p.rk >= 4 && !P.lim) return i + 1 < P.k ? c->kbuf(i) : c->q((P.A + 1) % 3);    // the step's result: buffer B
   return c->q(substep_out(P.A, i));
 }
 
@@ -421,7 +421,7 @@ StepPlan make_plan(const dg_ctx* c, double dt, double* stages) {
   P.damp = has_damping(c->p);
   P.lim = c->p.limiter != 0;
   P.fuse_tail = !stages && (c->fused_cfl || P.damp);   // damping + CFL ride on the step's last kernel
-  P.fast4 = c->p.rk == 4 && c->rk4_low_storage && c->ssp54.ok;
+  P.fast4 = c->p.rk == 4 && c->rk4_low_storage && c->ssp54.ok && !P.lim;   // see run_substep on the limiter
   P.dt = dt;
   P.stages = stages;
   return P;
@@ -459,15 +459,11 @@ int run_substep(dg_ctx* c, const StepPlan& P, int i) {
       // y_5 = (1 - alpha_4) u^n + alpha_4 y_4 + beta_4 dt L(y_4): no slope is ever stored
       const double r = S.d3 / S.beta[3];
       GenArgs ga{};
-      ga.kbase = S.c4 + r;    // base array: y_5 itself
-      ga.nk = 3;
+      ga.nk = 2;
       ga.kin[0] = c->q(Cc); ga.kc[0] = S.c2;
       ga.kin[1] = c->q(B); ga.kc[1] = S.c3 - r * S.alpha[3];
-      ga.kin[2] = c->q(P.A); ga.kc[2] = -r * (1.0 - S.alpha[3]);
-      ga.kself = S.d4;
-      ga.kout = nullptr;
       const int kind = (P.fuse_tail && !P.lim) ? K_GENL : K_GEN;
-      e = launch_stage(c, qin, qin, qout, 0.0, 0.0, dt, ts, kind, &ga);
+      e = launch_stage(c, qin, qn, qout, -r * (1.0 - S.alpha[3]), S.c4 + r, dt, ts, kind, &ga, S.d4);
     }
   } else if (c->p.rk <= 3) {
     // SSP-RK in Shu-Osher form, stage times c = (0,1) / (0,1,1/2)
@@ -477,19 +473,32 @@ int run_substep(dg_ctx* c, const StepPlan& P, int i) {
     else if (i == 1)             e = launch_stage(c, qin, qn, qout, 0.75, 0.25, dt, c->t + dt, K_MID);
     else                         e = launch_stage(c, qin, qn, qout, 1.0 / 3.0, 2.0 / 3.0, dt, c->t + 0.5 * dt, last_kind);
   } else {
-    // Butcher form (Appendix A): y_{i+1} = u^n + sum_{j<=i} a_{i+1,j} K_j, K_j = dt N(y_j, t_j),
-    // the last row being b.  Sub-step i reads y_i (with halo), u^n and the earlier K_j, writes K_i and y_{i+1}.
+    // General explicit scheme (Appendix A) in state form (dg_tables.h): sub-step i reads its
+    // input y_{i+1} (with halo), u^n and the earlier states with a non-zero coefficient, and writes y_{i+2}.
     ButcherTableau bt;
     butcher_tableau(c->p.rk, &bt);
-    const double* coef = last ? bt.b : bt.a[i + 1];
-    GenArgs ga{};
-    for (int j = 0; j < i; ++j)
-      if (coef[j] != 0.0) { ga.kin[ga.nk] = c->kbuf(j); ga.kc[ga.nk] = coef[j]; ga.nk++; }
-    ga.kself = coef[i];
-    ga.kout = last ? nullptr : c->kbuf(i);
-    // K_GENL fuses wave-killing + CFL; K_GEN never damps
-    const int kind = (last && P.fuse_tail && !P.lim) ? K_GENL : K_GEN;
-    e = launch_stage(c, qin, qn, qout, 0.0, 0.0, dt, c->t + bt.c[i] * dt, kind, &ga);
+    const double ts = c->t + bt.c[i] * dt;
+    if (P.lim) {
+      // The limiter changes every stage state after it is formed, so slopes cannot be recovered from states:
+      // keep Z_i = abar_i u^n + beta_i dt N(y_i) (spare buffer i) instead (dg_tables.h, ZForm).  Exactly the
+      // Butcher form with the limiter after every sub-step, as the oracle runs it.
+      const ZForm Z = z_form_from_butcher(bt);
+      GenArgs ga{};
+      for (int j = 0; j < i; ++j)
+        if (Z.z[i][j] != 0.0) { ga.kin[ga.nk] = c->kbuf(j); ga.kc[ga.nk] = Z.z[i][j]; ga.nk++; }
+      ga.zout = last ? nullptr : c->kbuf(i);
+      e = launch_stage(c, qin, qn, qout, Z.abar[i], 0.0, dt, ts, K_GEN, &ga, Z.beta[i]);
+    } else if (i == 0) {
+      const StateForm F = state_form_from_butcher(bt);
+      e = launch_stage(c, qin, qn, qout, 0.0, 1.0, dt, ts, K_FIRST, nullptr, F.beta[0]);
+    } else {
+      const StateForm F = state_form_from_butcher(bt);
+      GenArgs ga{};
+      for (int m = 1; m < i; ++m)               // y_{m+1}, m = 1..i-1, sits in spare buffer m-1
+        if (F.g[i][m] != 0.0) { ga.kin[ga.nk] = c->kbuf(m - 1); ga.kc[ga.nk] = F.g[i][m]; ga.nk++; }
+      const int kind = (last && P.fuse_tail) ? K_GENL : K_GEN;
+      e = launch_stage(c, qin, qn, qout, F.g[i][0], F.g[i][i], dt, ts, kind, &ga, F.beta[i]);
+    }
   }
   if (e) return e;
   if (P.lim && (e = launch_limit(c, qout, last && P.fuse_tail, dt))) return e;
@@ -504,6 +513,8 @@ int step_end(dg_ctx* c, const StepPlan& P) {
   if (P.fast4) {            // the new state sits in spare buffer 0: it becomes buffer A, the old u^n the spare
     std::swap(c->L.off_q[P.A], c->L.off_k[0]);
     c->cur = P.A;
+  } else if (c->p.rk >= 4 && !P.lim) {
+    c->cur = (P.A + 1) % 3;
   } else {
     c->cur = substep_out(P.A, P.k - 1);
   }

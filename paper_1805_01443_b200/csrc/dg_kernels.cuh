@@ -39,12 +39,12 @@ enum : int {          // KIND: what the epilogue of the stage does
   K_MID   = 2,        // a u^n + b (u + dt N)
   K_LAST  = 3,        // K_MID + fused CFL wave-speed reduction
   K_LASTD = 4,        // K_LAST + wave-killing relaxation
-  K_GEN   = 5,        // Butcher-form sub-step: K_i = dt N(y_i) -> kout,
-                      //   out = kbase u^n + sum_j kc[j] kin[j] + kself K_i
-  K_GENL  = 6,        // K_GEN of the last sub-step: no kout, fused CFL reduction, wave-killing if enabled
+  K_GEN   = 5,        // sub-step of a general explicit scheme (Appendix A) in state form
+                      //   (dg_tables.h): K_MID plus earlier stage states, out = a u^n + b u + sum_j kc[j] kin[j] + beta N
+  K_GENL  = 6,        // K_GEN of the last sub-step: fused CFL reduction, wave-killing if enabled
   K_COUNT = 7,
 };
-constexpr int MAXK = 5;   // earlier slopes a Butcher sub-step can read (Cash-Karp: 5)
+constexpr int MAXK = 5;   // earlier stage states a general sub-step can combine (Cash-Karp's last: 4)
 enum : int { G_NONE = 0, G_STAR = 1, G_PLANET = 2 };   // GRAV: gravity source terms present
 
 struct DevTables {            // kernel-parameter (constant bank) copy of the tables
@@ -112,13 +112,12 @@ struct StageArgs {
   double a, b, dt;            // out = a u^n + b u^(s-1) + beta N; beta = b dt is folded into T and ph
   DampArgs D;
   int rows;
-  // K_GEN / K_GENL: earlier slopes K_j = dt N(y_j) with their Butcher coefficients, this sub-step's own
-  // coefficient, and where to keep K_i (null: not needed again)
+  // K_GEN / K_GENL: the earlier stage states the sub-step combines (besides u^n and its input) and their
+  // coefficients
   const double* kin[MAXK];
   double kc[MAXK];
-  double kself;
-  double kbase;               // coefficient of the base array qn (1 in the Butcher form)
-  double* kout;
+  double* zout;               // if set: also store a u^n + b u + beta N, the value before the kin terms are added
+                              // (limiter runs keep these instead of stage states: the limiter changes the states)
   int nk;
   int gen_pf;                 // L2 prefetch of the epilogue's inputs: 0 none, 1 row start, 2 a row ahead (evicted before use: 1.7x DRAM reads), 3 at the x/y phase boundary
   Geom g;
@@ -362,8 +361,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   constexpr bool grav = GRAV != G_NONE;
   constexpr bool need_ri = EOS == 1 || grav;
   constexpr bool gen = KIND == K_GEN || KIND == K_GENL;
-  constexpr bool add_u = KIND != K_RHS && !gen;
-  constexpr bool use_un = KIND == K_MID || KIND == K_LAST || KIND == K_LASTD;
+  constexpr bool add_u = KIND != K_RHS;
+  constexpr bool use_un = KIND == K_MID || KIND == K_LAST || KIND == K_LASTD || gen;
   constexpr bool do_cfl = KIND == K_LAST || KIND == K_LASTD || KIND == K_GENL;
   constexpr bool do_damp = KIND == K_LASTD || KIND == K_GENL;    // K_GENL: only if the zone is enabled
   constexpr int C = 4 * M * M;                   // doubles per cell
@@ -451,10 +450,9 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     if (want) bulk_prefetch_l2(A.q0 + (size_t)j * row_stride + (size_t)ib * BS, TILE_BYTES);
   };
 
-  // Butcher sub-steps read u^n and the earlier slopes in the epilogue: pull the row's tiles into L2 ahead
-  auto prefetch_gen = [&](int j) {               // thread 0 only
+  // general sub-steps read earlier stage states in the epilogue: pull the row's tiles into L2 ahead
+  auto prefetch_gen = [&](int j) {               // issuing thread only
     const size_t off = (size_t)j * row_stride + (size_t)ib * BS;
-    bulk_prefetch_l2(A.qn + off, TILE_BYTES);
     for (int k = 0; k < A.nk; ++k) bulk_prefetch_l2(A.kin[k] + off, TILE_BYTES);
   };
 
@@ -775,12 +773,10 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
         double avg = 0.0;
-        // Butcher sub-step: u^n and the earlier slopes of this variable's column, all requested before the
-        // first use (independent loads in flight together; slots >= nk are predicated off)
-        double gb[M], gk[MAXK][M];
+        // general sub-step: the earlier stage states of this variable's column, all requested before the first
+        // use (independent loads in flight together; slots >= nk are predicated off)
+        double gk[MAXK][M];
         if (gen) {
-#pragma unroll
-          for (int rr = 0; rr < M; ++rr) gb[rr] = __ldg(A.qn + cell_off + ((v * M + rr) * M + q) * 32);
 #pragma unroll
           for (int k = 0; k < MAXK; ++k)
 #pragma unroll
@@ -792,13 +788,10 @@ stage_kernel(const __grid_constant__ StageArgs A) {
           const int e = ((v * M + rr) * M + q) * 32;
           double out = sN[e + lane] + acc[v][rr];
           out = fma(T.lym[rr], HS[v], fma(-T.lyp[rr], HN[v], out));
-          if (gen) {                               // out is K_i = dt N(y_i) here
-            const double K = out;
-            if (KIND == K_GEN && A.kout && valid) A.kout[cell_off + e] = K;
-            out = A.kbase * gb[rr];
+          if (gen) {
+            if (KIND == K_GEN && A.zout && valid) A.zout[cell_off + e] = out;
 #pragma unroll
             for (int k = 0; k < MAXK; ++k) out = fma(A.kc[k], gk[k][rr], out);   // kc = 0 beyond nk
-            out = fma(A.kself, K, out);
           }
           if (do_damp && damp) out = fma(f0, early_q0 ? z0[v][rr] : __ldg(A.q0 + cell_off + e), ft * out);
           if (valid) qo[e] = out;

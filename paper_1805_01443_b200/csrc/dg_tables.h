@@ -179,6 +179,61 @@ inline bool butcher_tableau(int rk, ButcherTableau* B) {
   return false;
 }
 
+// Any explicit scheme with non-zero sub-diagonal, rewritten on the stage STATES instead of the slopes: with
+// y_1 = u^n and K_j = dt L(y_j), the Butcher rows y_l = u^n + sum_{j<l} a_lj K_j (l = 2..s+1, row s+1 = b) give
+// K_j = (y_{j+1} - u^n - sum_{k<j} a_{j+1,k} K_k)/a_{j+1,j} recursively, hence
+//   y_{i+2} = sum_{m=0..i} g[i][m] y_{m+1} + beta[i] dt L(y_{i+1}),     i = 0..s-1,   beta[i] = a_{i+2,i+1}.
+// A sub-step then reads its input y_{i+1} (whose tile it holds anyway), u^n and the earlier states with
+// g != 0, and writes ONE array -- no slope is ever stored.  Same arithmetic up to rounding (the
+// reconstruction divides state differences of size dt |L| by a_{j+1,j}: errors of 1e-16 |y|).
+struct StateForm { int s; bool ok; double g[6][7], beta[6]; };
+
+inline StateForm state_form_from_butcher(const ButcherTableau& B) {
+  StateForm F{};
+  F.s = B.s;
+  F.ok = true;
+  double kap[6][7] = {};                       // K_j = sum_m kap[j][m] y_{m+1}
+  for (int i = 0; i < B.s; ++i) {
+    const double* row = (i + 1 < B.s) ? B.a[i + 1] : B.b;   // row of y_{i+2}
+    F.beta[i] = row[i];
+    if (row[i] == 0.0) F.ok = false;
+    for (int m = 0; m < 7; ++m) F.g[i][m] = 0.0;
+    F.g[i][0] = 1.0;
+    for (int j = 0; j < i; ++j)
+      for (int m = 0; m <= j + 1; ++m) F.g[i][m] += row[j] * kap[j][m];
+    // K_i from y_{i+2} = sum_m g[i][m] y_{m+1} + row[i] K_i
+    if (row[i] != 0.0) {
+      for (int m = 0; m <= i; ++m) kap[i][m] = -F.g[i][m] / row[i];
+      kap[i][i + 1] = 1.0 / row[i];
+    }
+  }
+  return F;
+}
+
+// The same scheme when a limiter modifies every y_l after it is formed: the slopes cannot be
+// recovered from the (limited) states, so each sub-step also keeps Z_i = abar_i u^n + beta_i K_i -- its result
+// before the earlier slopes' terms are added, which the limiter never touches.  With K_j = (Z_j - abar_j u^n)/beta_j,
+//   y_{i+2} = abar_i u^n + sum_{j<i} z[i][j] Z_j + beta_i K_i,  z[i][j] = row_i[j]/beta_j,  abar_i = 1 - sum_{j<i} z[i][j] abar_j.
+struct ZForm { int s; bool ok; double abar[6], z[6][6], beta[6]; };
+
+inline ZForm z_form_from_butcher(const ButcherTableau& B) {
+  ZForm F{};
+  F.s = B.s;
+  F.ok = true;
+  for (int i = 0; i < B.s; ++i) {
+    const double* row = (i + 1 < B.s) ? B.a[i + 1] : B.b;
+    F.beta[i] = row[i];
+    if (row[i] == 0.0 && i + 1 < B.s) F.ok = false;
+    double abar = 1.0;
+    for (int j = 0; j < i; ++j) {
+      F.z[i][j] = row[j] / F.beta[j];
+      abar -= F.z[i][j] * F.abar[j];
+    }
+    F.abar[i] = abar;
+  }
+  return F;
+}
+
 // Table 1's scheme in the low-storage (Shu-Osher) form it has by construction: rows 2..5 of the printed
 // tableau are multiples of the row above plus one new entry, a_{i+1,j} = alpha_i a_{ij} (j < i), so that
 //   y_{i+1} = (1 - alpha_i) u^n + alpha_i y_i + beta_i dt L(y_i),  i = 1..4  (alpha_1 = 1),

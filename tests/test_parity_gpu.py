@@ -340,7 +340,7 @@ def test_limiter_parity(DG, case):
     np.testing.assert_allclose(out[..., 0, 0], U[..., 0, 0], rtol=1e-14)
 
 
-@pytest.mark.parametrize("rk", [2, 3, 5])
+@pytest.mark.parametrize("rk", [2, 3, 4, 5])
 @pytest.mark.parametrize("case", NEXT_CASES[:5], ids=_id)
 def test_limited_step_parity(DG, case, rk):
     """A full step with the limiter after every sub-step, from a state the limiter has
