@@ -496,7 +496,8 @@ int run_substep(dg_ctx* c, const StepPlan& P, int i) {
       GenArgs ga{};
       for (int m = 1; m < i; ++m)               // y_{m+1}, m = 1..i-1, sits in spare buffer m-1
         if (F.g[i][m] != 0.0) { ga.kin[ga.nk] = c->kbuf(m - 1); ga.kc[ga.nk] = F.g[i][m]; ga.nk++; }
-      const int kind = (last && P.fuse_tail) ? K_GENL : K_GEN;
+      int kind = (last && P.fuse_tail) ? K_GENL : K_GEN;
+      if (ga.nk == 0) kind = kind == K_GEN ? K_MID : (P.damp ? K_LASTD : K_LAST);   // nothing to gather: the plain SSP stage
       e = launch_stage(c, qin, qn, qout, F.g[i][0], F.g[i][i], dt, ts, kind, &ga, F.beta[i]);
     }
   }
