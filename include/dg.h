@@ -34,7 +34,7 @@ extern "C" {
 #define DG_OK       0
 #define DG_EINVAL  (-1)   /* bad parameter, null or misaligned pointer */
 #define DG_ENOSPC  (-2)   /* workspace too small */
-#define DG_ESTATE  (-3)   /* state not set yet */
+#define DG_ESTATE  (-3)   /* state not set yet, or the call is not allowed between dg_step_begin and dg_step_end */
 #define DG_ECUDA   (-4)   /* CUDA runtime / launch error (message in dg_last_error) */
 
 typedef struct dg_ctx dg_ctx;     /* opaque, host-side, owned by the library */
@@ -76,6 +76,9 @@ typedef struct {
                                      one-sub-domain-per-GPU design): the rows below y0 / above y1
                                      belong to a neighbour strip and are read from a halo row the caller fills before
                                      every sub-step (dg_halo_layout), instead of applying `bc` at that edge */
+  int32_t damp_mode;              /* fields the wave-killing zones relax: 0 the conservative state
+                                     (reading G13); 1 "the density, velocities and temperature"
+                                     at the m x m Gauss points, conservative state rebuilt from them (reading D2) */
 } dg_params;
 
 /* Bytes of DEVICE workspace dg_init needs for these parameters (0 if they are invalid). */
@@ -119,6 +122,9 @@ int dg_step(dg_ctx*, double dt);
 int dg_step_begin(dg_ctx*, double dt);
 int dg_substep(dg_ctx*);
 int dg_step_end(dg_ctx*);
+/* Between dg_step_begin and dg_step_end the workspace's spare state buffers hold live sub-step data: dg_rhs,
+ * dg_get_state*, dg_limit, dg_cfl_dt, dg_torque*, dg_step and dg_step_debug return DG_ESTATE there (they use those
+ * buffers as scratch, or would act on a state that is not a time level).  dg_set_state* abandons the split step. */
 
 /* Where the halo exchange reads and writes, as byte offsets into the workspace given to dg_init (internal
  * layout, one row of cells = *row_bytes contiguous bytes): offsets[0], [1] = first and last row of the array
@@ -150,6 +156,12 @@ int dg_limit(dg_ctx*);
  * M_n = cell-average density x cell area, r_n = cell centre, G = gm_star (unit stellar mass).
  * Synchronises the stream and writes one HOST double. */
 int dg_torque(dg_ctx*, double t, double* gamma_z /*HOST*/);
+
+/* The torque as the paper quotes it: gamma Gamma / Gamma_0 with Gamma_0 = Sigma Omega^2 r_p^4 q / h^2,
+ * Sigma = sigma_p (the unperturbed surface density at the planet's orbit: a property of the caller's initial data),
+ * Omega = omega_planet, q = q_planet, h = h_aspect, gamma = the adiabatic index.  DG_EINVAL without a planet or
+ * with h_aspect <= 0.  Synchronises the stream and writes one HOST double. */
+int dg_torque_normalised(dg_ctx*, double t, double sigma_p, double* out /*HOST*/);
 
 /* Convenience for end-to-end runs from HOST buffers: set_state_host(U_in), then nsteps times
  * { dg_cfl_dt(cfl); dg_step(dt) }, then get_state_host(U_out).  Blocking. */

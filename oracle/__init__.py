@@ -45,6 +45,7 @@ class RefParams(C.Structure):
         ("limiter", C.c_int32), ("lim_eps", C.c_double),
         ("flux", C.c_int32),
         ("damp_in_r0", C.c_double), ("damp_in_r1", C.c_double),
+        ("damp_mode", C.c_int32),
     ]
 
 
@@ -80,9 +81,11 @@ def _lib(omp: bool):
         "ref_hllc": (i, [PP, _PD, _PD, d, d, i, _PD]),
         "ref_gravity": (i, [PP, d, d, d, _PD]),
         "ref_rhs_parts": (i, [vp, d, i, _PD]), "ref_damp": (i, [vp, d]),
+        "ref_load_working_state": (i, [vp, _PD]),
         "ref_rk_step": (i, [i, C.c_long, _PD, d, d, _ODE_FN, vp, _PD]),
         "ref_threads": (i, []), "ref_set_threads": (None, [i]),
         "ref_rk_stages": (i, [i]), "ref_limit": (i, [vp]), "ref_torque": (i, [vp, d, _PD]),
+        "ref_torque_normalised": (i, [vp, d, d, _PD]),
         "ref_lobatto": (i, [i, _PD, _PD]), "ref_limit_cell": (i, [PP, _PD, _PD]),
     }
     for name, (res, args) in sig.items():
@@ -135,6 +138,12 @@ class RefDG:
         assert U.shape == self.shape
         _chk(self.L.ref_set_state(self._h, _p(U)), "ref_set_state")
 
+    def load_working_state(self, U: np.ndarray):
+        """Replace the working state; the snapshot U0 taken by set_state stays."""
+        U = np.ascontiguousarray(U, dtype=np.float64)
+        assert U.shape == self.shape
+        _chk(self.L.ref_load_working_state(self._h, _p(U)), "ref_load_working_state")
+
     def get_state(self) -> np.ndarray:
         U = np.empty(self.shape)
         _chk(self.L.ref_get_state(self._h, _p(U)), "ref_get_state")
@@ -164,6 +173,12 @@ class RefDG:
     def torque(self, t: float) -> float:
         g = C.c_double()
         _chk(self.L.ref_torque(self._h, float(t), C.byref(g)), "ref_torque")
+        return g.value
+
+    def torque_normalised(self, t: float, sigma_p: float) -> float:
+        """gamma Gamma / Gamma_0."""
+        g = C.c_double()
+        _chk(self.L.ref_torque_normalised(self._h, float(t), float(sigma_p), C.byref(g)), "ref_torque_normalised")
         return g.value
 
     def damp(self, dt: float):

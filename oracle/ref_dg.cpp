@@ -15,7 +15,7 @@
  *   C11 wave damping
  *   C8b Butcher-form RK PAPER.md:445-457 (Appendix A), Table 1, Table 2
  *   C12 positivity limiter  PAPER.md:129-131, 150 (Zhang & Shu 2010; readings L1..L5 in DESIGN.md)
- *   C13 torque on the planet  PAPER.md:321-328  Eq.(6)
+ *   C13 torque on the planet  PAPER.md:321-328  Eq.(6); C13b its normalisation gamma Gamma/Gamma_0
  *
  * No blocking, fusion, sum-factorisation or reordering: every sum is written as the nested loop
  * the formula states, in fp64, compiled with -O2 -ffp-contract=off.
@@ -30,7 +30,10 @@
  *   C6+C7  Keplerian equilibrium residual -> 0 at rate h^(p+1)
  *   C8  y' = lambda y observed order 2 / 3; exact on polynomials of degree <= order
  *   C7+C8  isentropic-vortex L1 error slope ~ p+1
- *   C10 hand value on a constant state;  C11 R = 0 identity, fixed point, tau -> 0 limit
+ *   C10 hand value on a constant state;  C11 R = 0 identity, fixed point, tau -> 0 limit; damp_mode 1: node-wise
+ *       relation of the primitive fields through NumPy's basis evaluation, a hand-worked constant cell
+ *   C9  frozen boundary: = transmissive before the state moves; NumPy traces of U / U0 afterwards
+ *   C4  eos 1 on faces: m-point quadrature of the point-wise flux with c_s at the face nodes
  *   C8b the tableaus against the paper's printed digits (tests/golden/rk_tableaus.txt), row sums = c,
  *       order conditions, observed order 4 / 5 on y' = lambda y and on a non-autonomous ODE
  *   C12 Gauss-Lobatto closed forms and exactness; the cell average as a convex combination of the
@@ -384,7 +387,53 @@ void dg_ode(void* user, double t, const double* y, double* dydt) {
 
 /* C11: Q <- (dt Q0 + tau Q)/(tau + dt), tau = 2 pi sqrt(r_d^3/GM)/R(r), R(r) = ((r - r_d)/(r_b - r_d))^2
  * clamped to 1 beyond the boundary radius r_b.  Outer zone: r_d = damp_r0 < r,
- * r_b = damp_r1; inner zone (the paper's own disc): r_d = damp_in_r0 > r, r_b = damp_in_r1. */
+ * r_b = damp_r1; inner zone (the paper's own disc): r_d = damp_in_r0 > r, r_b = damp_in_r1.  r = the cell centre.
+ * damp_mode 0 (reading G13): Q runs over the conservative modal coefficients.
+ * damp_mode 1 ("The dampened fields are the density, velocities and temperature"; reading D2):
+ * at each of the cell's m x m Gauss points (C2) Q runs over rho, v_x = m_x/rho, v_y = m_y/rho and T = p/rho
+ * (p from Eq.(2), of the carried energy for either closure), Q0 over the same fields of the initial
+ * state; the conservative state (rho, rho v, rho T/(gamma-1) + rho v^2/2) rebuilt from the relaxed fields is
+ * projected back onto the modes with the m-point rule, which is exact here. */
+void damp_cell_primitive(const ref_ctx* c, double f0, double ft, double* u, const double* u0) {
+  const int mo = c->m;                               /* order (m[] below are a node's conservative values) */
+  const Tables& T = c->T;
+  const double gm1 = c->p.gamma - 1.0;
+  double nod[MAXM][MAXM][NV];
+  for (int r = 0; r < mo; ++r)
+    for (int q = 0; q < mo; ++q) {
+      double m[NV], m0[NV];                          /* C2: nodal values of U and of the initial state U0 */
+      for (int v = 0; v < NV; ++v) {
+        double s = 0.0, s0 = 0.0;
+        for (int b = 0; b < mo; ++b)
+          for (int a = 0; a < mo; ++a) {
+            s += u[(v * mo + b) * mo + a] * T.B[q][a] * T.B[r][b];
+            s0 += u0[(v * mo + b) * mo + a] * T.B[q][a] * T.B[r][b];
+          }
+        m[v] = s; m0[v] = s0;
+      }
+      const double r0 = m0[0], v0x = m0[1] / m0[0], v0y = m0[2] / m0[0];
+      const double pr0 = gm1 * (m0[3] - 0.5 * (m0[1] * m0[1] + m0[2] * m0[2]) / m0[0]);
+      const double T0 = pr0 / r0;
+      const double pr = gm1 * (m[3] - 0.5 * (m[1] * m[1] + m[2] * m[2]) / m[0]);
+      const double rho = f0 * r0 + ft * m[0];
+      const double vx = f0 * v0x + ft * (m[1] / m[0]);
+      const double vy = f0 * v0y + ft * (m[2] / m[0]);
+      const double T = f0 * T0 + ft * (pr / m[0]);
+      nod[q][r][0] = rho;
+      nod[q][r][1] = rho * vx;
+      nod[q][r][2] = rho * vy;
+      nod[q][r][3] = rho * T / gm1 + 0.5 * rho * (vx * vx + vy * vy);
+    }
+  for (int v = 0; v < NV; ++v)
+    for (int b = 0; b < mo; ++b)
+      for (int a = 0; a < mo; ++a) {
+        double s = 0.0;
+        for (int q = 0; q < mo; ++q)
+          for (int r = 0; r < mo; ++r) s += T.w[q] * T.w[r] * nod[q][r][v] * T.B[q][a] * T.B[r][b];
+        u[(v * mo + b) * mo + a] = 0.25 * s;
+      }
+}
+
 void damp(ref_ctx* c, double dt) {
   const ref_params& p = c->p;
   if (!(p.damp_r0 > 0.0) && !(p.damp_in_r0 > 0.0)) return;
@@ -410,7 +459,8 @@ void damp(ref_ctx* c, double dt) {
       const double tau = 2.0 * pi * std::sqrt(rd * rd * rd / p.gm_star) / R;
       double* u = c->U.data() + cell_off(c, i, j);
       const double* u0 = c->U0.data() + cell_off(c, i, j);
-      for (int k = 0; k < NV * m * m; ++k) u[k] = (dt * u0[k] + tau * u[k]) / (tau + dt);
+      if (p.damp_mode == 1) damp_cell_primitive(c, dt / (tau + dt), tau / (tau + dt), u, u0);
+      else for (int k = 0; k < NV * m * m; ++k) u[k] = (dt * u0[k] + tau * u[k]) / (tau + dt);
     }
 }
 
@@ -612,6 +662,7 @@ int check_params(const ref_params* p) {
   if (p->flux != 0 && p->flux != 1) return -1;
   if (p->limiter == 1 && !(p->lim_eps > 0.0)) return -1;
   if (p->damp_in_r0 > 0.0 && !(p->damp_in_r1 >= 0.0 && p->damp_in_r1 < p->damp_in_r0 && p->gm_star > 0.0)) return -1;
+  if (p->damp_mode != 0 && p->damp_mode != 1) return -1;
   return 0;
 }
 
@@ -640,6 +691,12 @@ int ref_set_state(ref_ctx* c, const double* U) {
   c->U.assign(U, U + c->ncoef);
   c->U0 = c->U;
   c->has_state = true;
+  return 0;
+}
+
+int ref_load_working_state(ref_ctx* c, const double* U) {
+  if (!c || !U || !c->has_state) return -1;
+  c->U.assign(U, U + c->ncoef);
   return 0;
 }
 
@@ -783,6 +840,18 @@ int ref_torque(ref_ctx* c, double t, double* gamma_z) {
     }
   (void)m;
   *gamma_z = xp * ay - yp * ax;
+  return 0;
+}
+
+/* C13b: the quantity the paper plots, gamma Gamma / Gamma_0 with Gamma_0 = Sigma Omega^2 r_p^4 q / h^2 */
+int ref_torque_normalised(ref_ctx* c, double t, double sigma_p, double* out) {
+  if (!c || !out || !(c->p.q_planet > 0.0) || !(c->p.h_aspect > 0.0)) return -1;
+  double g;
+  if (ref_torque(c, t, &g) != 0) return -1;
+  const ref_params& p = c->p;
+  const double rp2 = p.r_planet * p.r_planet;
+  const double gamma0 = sigma_p * p.omega_planet * p.omega_planet * rp2 * rp2 * p.q_planet / (p.h_aspect * p.h_aspect);
+  *out = p.gamma * g / gamma0;
   return 0;
 }
 

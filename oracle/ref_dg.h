@@ -42,6 +42,9 @@ typedef struct {
                                 1 HLLC (eos 0; Toro, Spruce & Speares 1994) / HLL (eos 1), Davis wave speeds (C5b) */
   double  damp_in_r0, damp_in_r1; /* inner wave-killing zone r < damp_in_r0 (r_d = r_in 1.15^(3/2),
                                      boundary radius r_in = damp_in_r1); damp_in_r0 <= 0: off */
+  int32_t damp_mode;         /* which fields the wave-killing zones relax (C11): 0 the conservative coefficients
+                                (reading G13); 1 "the density, velocities and temperature" at the
+                                m x m Gauss points, the conservative state rebuilt from them (reading D2) */
 } ref_params;
 
 /* --- the same surface as include/dg.h, prefixed ref_, host memory --- */
@@ -55,6 +58,9 @@ int    ref_step_debug(ref_ctx*, double dt, double* stages); /* also u^(1..k), be
 int    ref_rk_stages(int rk);                      /* sub-steps of the scheme: 2, 3, 5 (rk 4), 6 (rk 5) */
 int    ref_limit(ref_ctx*);                        /* C12 alone: limit the current state in place */
 int    ref_torque(ref_ctx*, double t, double* gamma_z); /* C13: Eq.(6) */
+/* C13b: gamma Gamma / Gamma_0, Gamma_0 = Sigma Omega^2 r_p^4 q / h^2; Sigma = sigma_p, the unperturbed
+ * surface density at the planet (a property of the initial data, passed in), Omega = omega_planet, h = h_aspect */
+int    ref_torque_normalised(ref_ctx*, double t, double sigma_p, double* out);
 double ref_time(const ref_ctx*);
 int    ref_set_time(ref_ctx*, double t);
 void   ref_destroy(ref_ctx*);
@@ -77,6 +83,8 @@ int  ref_gravity(const ref_params*, double t, double x, double y, double* g2);
 int  ref_rhs_parts(ref_ctx*, double t, int parts, double* L);
 /* C11 alone. */
 int  ref_damp(ref_ctx*, double dt);
+/* replaces the working state and leaves the snapshot U0 of the last ref_set_state alone (pins of C9, C11) */
+int  ref_load_working_state(ref_ctx*, const double* U);
 /* C12 pieces: Gauss-Lobatto nodes on [-1,1] and weights normalised to sum 1 (Zhang & Shu's hat-w)
  * for the limiter of order m (nh = ceil((m+2)/2) points); returns nh.  xh, wh sized 4. */
 int  ref_lobatto(int m, double* xh, double* wh);

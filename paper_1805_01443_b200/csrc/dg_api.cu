@@ -28,7 +28,10 @@ struct Layout {
   size_t state_doubles;      // ny * nbx * 4 m^2 * 32
   size_t state_bytes;
   bool need_q0, need_btr;
-  int nkbuf;                 // slope buffers K_j of the Butcher-form schemes (rk 4: 4, rk 5: 5)
+  int nkbuf;                 // spare state buffers of the general schemes inside `total` (rk 5: 5; rk 4: 2 for the
+                             // low-storage form, 4 with the limiter's Z form)
+  int nkbuf_opt;             // rk 4, limiter off: two more, past `total`, that only the generic state form
+                             // (DG_TUNE_RK4_FORM = 0) needs -- present if the caller's workspace is that large
   size_t row_bytes;          // one row of tiles: nbx * 4 m^2 * 32 doubles
   size_t off_haloS, off_haloN;
   size_t off_q[3], off_k[MAXK], off_q0, off_btrW, off_btrE, off_btrS, off_btrN, off_partial, off_scalars, total;
@@ -52,6 +55,8 @@ bool valid_params(const dg_params* p) {
   if (p->damp_in_r0 > 0.0 && !(p->damp_in_r1 >= 0.0 && p->damp_in_r1 < p->damp_in_r0 && p->gm_star > 0.0)) return false;
   if (p->damp_in_r0 > 0.0 && p->damp_r0 > 0.0 && !(p->damp_in_r0 <= p->damp_r0)) return false;
   if (p->gm_star < 0.0 || p->q_planet < 0.0) return false;
+  if (p->damp_mode != 0 && p->damp_mode != 1) return false;
+  if (p->damp_mode == 1 && !(p->gamma > 1.0)) return false;        // T = p/rho from Eq.(2)
   return true;
 }
 
@@ -65,7 +70,8 @@ Layout make_layout(const dg_params* p) {
   L.need_btr = p->bc == 2;
   size_t off = 0;
   for (int k = 0; k < 3; ++k) { L.off_q[k] = off; off += L.state_bytes; }
-  L.nkbuf = p->rk == 4 ? 4 : (p->rk == 5 ? 5 : 0);
+  L.nkbuf = p->rk == 4 ? (p->limiter ? 4 : 2) : (p->rk == 5 ? 5 : 0);
+  L.nkbuf_opt = (p->rk == 4 && !p->limiter) ? 2 : 0;
   for (int k = 0; k < MAXK; ++k) { L.off_k[k] = off; if (k < L.nkbuf) off += L.state_bytes; }
   L.off_q0 = off;
   if (L.need_q0) off += L.state_bytes;
@@ -82,6 +88,7 @@ Layout make_layout(const dg_params* p) {
   L.off_partial = off; off += align_up((size_t)L.nbx * ((p->ny + 3) / 4) * 2 * sizeof(double));
   L.off_scalars = off; off += ALIGN;
   L.total = off;
+  for (int k = 0; k < L.nkbuf_opt; ++k) L.off_k[L.nkbuf + k] = off + (size_t)k * L.state_bytes;   // past `total`
   return L;
 }
 }  // namespace
@@ -97,6 +104,7 @@ struct dg_ctx {
   Geom g;
   cudaStream_t stream;
   char* ws;
+  size_t ws_bytes;
   int cur;                    // index of the buffer holding u^n
   bool has_state;
   bool wmax_valid;            // the fused reduction of the last step matches the current state
@@ -182,6 +190,8 @@ DampArgs make_damp(const dg_ctx* c, double dt, bool enable = true) {
   D.dt = dt;
   D.r0 = INFINITY;
   D.on = enable && has_damping(p);
+  D.mode = p.damp_mode;
+  D.gm1 = p.gamma - 1.0;
   if (enable && p.damp_r0 > 0.0) {
     D.r0 = p.damp_r0;
     D.inv_w = 1.0 / (p.damp_r1 - p.damp_r0);
@@ -371,7 +381,14 @@ int launch_limit(dg_ctx* c, double* Q, bool final_, double dt) {
     constexpr int M = decltype(tag)::value;
     constexpr size_t smem = limit_smem_bytes<M>();
     auto go = [&](auto kern) {
-      err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      static std::atomic<bool> attr_set[kMaxDevices];      // per kernel instantiation (the lambda is), per device
+      int dev = 0;
+      err = cudaGetDevice(&dev);
+      const bool cached = dev >= 0 && dev < kMaxDevices;
+      if (err == cudaSuccess && (!cached || !attr_set[dev].load(std::memory_order_acquire))) {
+        err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (err == cudaSuccess && cached) attr_set[dev].store(true, std::memory_order_release);
+      }
       if (err == cudaSuccess) kern<<<grid, M * 32, smem, s>>>(A);
     };
     if (eos == 0) { if (final_) go(limit_kernel<M, 0, true>); else go(limit_kernel<M, 0, false>); }
@@ -421,6 +438,10 @@ StepPlan make_plan(const dg_ctx* c, double dt, double* stages) {
   P.damp = has_damping(c->p);
   P.lim = c->p.limiter != 0;
   P.fuse_tail = !stages && (c->fused_cfl || P.damp);   // damping + CFL ride on the step's last kernel
+  // the stage kernel's fused wave-killing relaxes the conservative state; "density, velocities, temperature"
+  // (damp_mode 1) needs all four variables of a node at once: the limiter's last pass does it
+  // (limiter on), else damp_kernel runs as its own pass after the last stage
+  if (P.damp && c->p.damp_mode == 1 && !P.lim) P.fuse_tail = false;
   P.fast4 = c->p.rk == 4 && c->rk4_low_storage && c->ssp54.ok && !P.lim;   // see run_substep on the limiter
   P.dt = dt;
   P.stages = stages;
@@ -566,6 +587,7 @@ int dg_init(const dg_params* p, void* workspace, size_t ws_bytes, void* cuda_str
   c->L = L;
   c->stream = static_cast<cudaStream_t>(cuda_stream);
   c->ws = static_cast<char*>(workspace);
+  c->ws_bytes = ws_bytes;
   c->cur = 0;
   c->has_state = false;
   c->wmax_valid = false;
@@ -587,6 +609,10 @@ int dg_init(const dg_params* p, void* workspace, size_t ws_bytes, void* cuda_str
     ButcherTableau bt;
     butcher_tableau(4, &bt);
     c->ssp54 = ssp54_from_butcher(bt);
+    if (!c->ssp54.ok && L.nkbuf_opt > 0 && ws_bytes < L.total + (size_t)L.nkbuf_opt * L.state_bytes) {
+      delete c;                                  // (cannot happen with the printed Table 1: it has the low-storage structure)
+      return DG_ENOSPC;
+    }
   }
   c->step_active = false;
   c->step_next = 0;
@@ -647,12 +673,14 @@ int dg_set_state_host(dg_ctx* c, const double* U) {
 int dg_get_state(dg_ctx* c, double* U) {
   if (!c || !U) return c ? fail(c, DG_EINVAL, "dg_get_state: null") : DG_EINVAL;
   if (!c->has_state) return fail(c, DG_ESTATE, "dg_get_state: state not set");
+  if (c->step_active) return fail(c, DG_ESTATE, "dg_get_state: a split step (dg_step_begin) is in progress");
   return to_modal(c, c->q(c->cur), U);
 }
 
 int dg_get_state_host(dg_ctx* c, double* U) {
   if (!c || !U) return c ? fail(c, DG_EINVAL, "dg_get_state_host: null") : DG_EINVAL;
   if (!c->has_state) return fail(c, DG_ESTATE, "dg_get_state_host: state not set");
+  if (c->step_active) return fail(c, DG_ESTATE, "dg_get_state_host: a split step (dg_step_begin) is in progress");
   const size_t bytes = (size_t)c->p.ny * c->p.nx * 4 * c->L.m * c->L.m * sizeof(double);
   double* staging = c->q((c->cur + 1) % 3);
   int e = to_modal(c, c->q(c->cur), staging);
@@ -665,6 +693,7 @@ int dg_get_state_host(dg_ctx* c, double* U) {
 int dg_rhs(dg_ctx* c, double t, double* Lout) {
   if (!c || !Lout) return c ? fail(c, DG_EINVAL, "dg_rhs: null") : DG_EINVAL;
   if (!c->has_state) return fail(c, DG_ESTATE, "dg_rhs: state not set");
+  if (c->step_active) return fail(c, DG_ESTATE, "dg_rhs: a split step (dg_step_begin) is in progress");
   double* scratch = c->q((c->cur + 1) % 3);
   int e = launch_stage(c, c->q(c->cur), c->q(c->cur), scratch, 0.0, 1.0, 0.0, t, K_RHS);
   if (e) return e;
@@ -674,6 +703,7 @@ int dg_rhs(dg_ctx* c, double t, double* Lout) {
 int dg_cfl_dt(dg_ctx* c, double cfl, double* dt) {
   if (!c || !dt) return c ? fail(c, DG_EINVAL, "dg_cfl_dt: null") : DG_EINVAL;
   if (!c->has_state) return fail(c, DG_ESTATE, "dg_cfl_dt: state not set");
+  if (c->step_active) return fail(c, DG_ESTATE, "dg_cfl_dt: a split step (dg_step_begin) is in progress");
   if (!c->wmax_valid) {
     CUDA_TRY(c, cudaMemsetAsync(c->wmax(), 0, sizeof(unsigned long long), c->stream));
     dim3 grid(c->L.nbx, (c->p.ny + 3) / 4);
@@ -707,6 +737,7 @@ int dg_rk_stages(int rk) { return rk == 2 ? 2 : rk == 3 ? 3 : rk == 4 ? 5 : rk =
 int dg_limit(dg_ctx* c) {
   if (!c) return DG_EINVAL;
   if (!c->has_state) return fail(c, DG_ESTATE, "dg_limit: state not set");
+  if (c->step_active) return fail(c, DG_ESTATE, "dg_limit: a split step (dg_step_begin) is in progress");
   c->wmax_valid = false;
   return launch_limit(c, c->q(c->cur), false, 0.0);
 }
@@ -714,6 +745,7 @@ int dg_limit(dg_ctx* c) {
 int dg_torque(dg_ctx* c, double t, double* gamma_z) {
   if (!c || !gamma_z) return c ? fail(c, DG_EINVAL, "dg_torque: null") : DG_EINVAL;
   if (!c->has_state) return fail(c, DG_ESTATE, "dg_torque: state not set");
+  if (c->step_active) return fail(c, DG_ESTATE, "dg_torque: a split step (dg_step_begin) is in progress");
   const Phys ph = make_phys(c, t);
   dim3 grid(c->L.nbx, (c->p.ny + 3) / 4);
   const int nblocks = (int)(grid.x * grid.y);
@@ -731,6 +763,20 @@ int dg_torque(dg_ctx* c, double t, double* gamma_z) {
   CUDA_TRY(c, cudaMemcpyAsync(res, out, sizeof res, cudaMemcpyDeviceToHost, c->stream));
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   *gamma_z = res[0];
+  return DG_OK;
+}
+
+int dg_torque_normalised(dg_ctx* c, double t, double sigma_p, double* out) {
+  if (!c || !out) return c ? fail(c, DG_EINVAL, "dg_torque_normalised: null") : DG_EINVAL;
+  const dg_params& p = c->p;
+  if (!(p.q_planet > 0.0) || !(p.h_aspect > 0.0) || !(sigma_p > 0.0))
+    return fail(c, DG_EINVAL, "dg_torque_normalised: needs a planet, h_aspect > 0 and sigma_p > 0");
+  double g = 0.0;
+  int e = dg_torque(c, t, &g);
+  if (e) return e;
+  const double rp2 = p.r_planet * p.r_planet;
+  const double gamma0 = sigma_p * p.omega_planet * p.omega_planet * rp2 * rp2 * p.q_planet / (p.h_aspect * p.h_aspect);
+  *out = p.gamma * g / gamma0;
   return DG_OK;
 }
 
@@ -827,6 +873,10 @@ int dg_set_tuning(dg_ctx* c, int key, int value) {
       return DG_OK;
     case DG_TUNE_RK4_FORM:
       if (c->step_active) return fail(c, DG_ESTATE, "a split step is in progress");
+      if (!value && c->ws_bytes < c->L.total + (size_t)c->L.nkbuf_opt * c->L.state_bytes) {
+        c->err = "the generic rk 4 form needs a workspace of dg_workspace_bytes() + 2 state arrays";
+        return DG_ENOSPC;
+      }
       c->rk4_low_storage = value ? 1 : 0;
       return DG_OK;
     case DG_TUNE_GEN_PREFETCH:

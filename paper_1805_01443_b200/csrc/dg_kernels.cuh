@@ -77,6 +77,8 @@ struct DampArgs {
   double r0, inv_w, tau0;          // outer: r_d, 1/(r_b - r_d), 2 pi sqrt(r_d^3/GM); off: r0 = +inf, on = 0
   double in_r0, in_inv_w, in_tau0; // inner: r_d, 1/(r_d - r_b), 2 pi sqrt(r_d^3/GM); off: in_r0 = 0
   int on;                          // any zone enabled
+  int mode;                        // 0: relax the conservative state; 1: density, velocities, temperature
+  double gm1;                      // gamma - 1 (mode 1: T = p/rho with p from Eq.(2))
   double dt;
 };
 __device__ __forceinline__ double rcp_fast(double x);
@@ -124,6 +126,23 @@ struct StageArgs {
   Phys ph;
   DevTables T;
 };
+
+// Wave-killing of "the density, velocities and temperature" (damp_mode 1) at one node: Q <- f0 Q0 + ft Q
+// for Q = rho, v_x, v_y, T = p/rho (p from Eq.(2) of the carried energy), then the conservative state of the
+// relaxed fields.  u: the node's current state (in/out), u0: the initial state's.
+__device__ __forceinline__ void damp_node_primitive(double f0, double ft, double gm1, double (&u)[4], const double (&u0)[4]) {
+  const double ri0 = 1.0 / u0[0], ri = 1.0 / u[0];
+  const double v0x = u0[1] * ri0, v0y = u0[2] * ri0, vx_ = u[1] * ri, vy_ = u[2] * ri;
+  const double T0 = gm1 * (u0[3] - 0.5 * (u0[1] * v0x + u0[2] * v0y)) * ri0;
+  const double T1 = gm1 * (u[3] - 0.5 * (u[1] * vx_ + u[2] * vy_)) * ri;
+  const double rho = fma(f0, u0[0], ft * u[0]);
+  const double vx = fma(f0, v0x, ft * vx_), vy = fma(f0, v0y, ft * vy_);
+  const double T = fma(f0, T0, ft * T1);
+  u[0] = rho;
+  u[1] = rho * vx;
+  u[2] = rho * vy;
+  u[3] = rho * (T / gm1 + 0.5 * (vx * vx + vy * vy));
+}
 
 // ---------------------------------------------------------------------------------------------
 // fp64 special functions without slow paths: MUFU seed (~20 bits) + 2 Newton steps (measured max
@@ -1021,6 +1040,18 @@ damp_kernel(double* __restrict__ Q, const double* __restrict__ Q0, Geom g, DampA
   double f0, ft;
   if (!damp_factors(D, sqrt(xc * xc + yc * yc), f0, ft)) return;
   const size_t base = ((size_t)j * g.nbx + ib) * C * 32 + lane;
+  if (D.mode == 1) {
+#pragma unroll 1
+    for (int n = 0; n < M * M; ++n) {
+      double u[4], u0[4];
+#pragma unroll
+      for (int v = 0; v < 4; ++v) { u[v] = Q[base + (v * M * M + n) * 32]; u0[v] = Q0[base + (v * M * M + n) * 32]; }
+      damp_node_primitive(f0, ft, D.gm1, u, u0);
+#pragma unroll
+      for (int v = 0; v < 4; ++v) Q[base + (v * M * M + n) * 32] = u[v];
+    }
+    return;
+  }
 #pragma unroll 4
   for (int e = 0; e < C; ++e) Q[base + e * 32] = fma(f0, Q0[base + e * 32], ft * Q[base + e * 32]);
 }

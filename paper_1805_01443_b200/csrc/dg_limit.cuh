@@ -216,20 +216,47 @@ limit_kernel(const __grid_constant__ LimitArgs A) {
     }
     const double* p0 = A.q0 + (size_t)j * row_stride + (size_t)ib * BS + lane;
     // (every thread read sAvg before the barrier that follows the sMin exchange: it may be rewritten now)
-#pragma unroll
-    for (int v = 0; v < 4; ++v) {
-      const double th = v == 0 ? th1 * th2 : th2;
-      double avg = 0.0;
+    if (FINAL && damp && A.D.mode == 1) {
+      // wave-killing of density, velocities and temperature: node by node over this thread's column
 #pragma unroll
       for (int r = 0; r < M; ++r) {
-        const int e = ((v * M + r) * M + w) * 32;
-        double val = uc[v][r];
-        if (changed) val = fma(th, val - ub[v], ub[v]);
-        if (damp) val = fma(f0, __ldg(p0 + e), ft * val);
-        if (valid && (changed || damp)) p[e] = val;
-        if (FINAL) avg = fma(LT.w[r], val, avg);
+        double u[4], u0[4];
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          const double th = v == 0 ? th1 * th2 : th2;
+          u[v] = changed ? fma(th, uc[v][r] - ub[v], ub[v]) : uc[v][r];
+          u0[v] = __ldg(p0 + ((v * M + r) * M + w) * 32);
+        }
+        damp_node_primitive(f0, ft, A.D.gm1, u, u0);
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          uc[v][r] = u[v];
+          if (valid) p[((v * M + r) * M + w) * 32] = u[v];
+        }
       }
-      if (FINAL) sAvg[(v * M + w) * 32 + lane] = 0.25 * LT.w[w] * avg;
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        double avg = 0.0;
+#pragma unroll
+        for (int r = 0; r < M; ++r) avg = fma(LT.w[r], uc[v][r], avg);
+        sAvg[(v * M + w) * 32 + lane] = 0.25 * LT.w[w] * avg;
+      }
+    } else {
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        const double th = v == 0 ? th1 * th2 : th2;
+        double avg = 0.0;
+#pragma unroll
+        for (int r = 0; r < M; ++r) {
+          const int e = ((v * M + r) * M + w) * 32;
+          double val = uc[v][r];
+          if (changed) val = fma(th, val - ub[v], ub[v]);
+          if (damp) val = fma(f0, __ldg(p0 + e), ft * val);
+          if (valid && (changed || damp)) p[e] = val;
+          if (FINAL) avg = fma(LT.w[r], val, avg);
+        }
+        if (FINAL) sAvg[(v * M + w) * 32 + lane] = 0.25 * LT.w[w] * avg;
+      }
     }
     if (FINAL) __syncthreads();                  // sAvg of this row complete (read by warp 0 next iteration)
   }

@@ -3,6 +3,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include "dg_tables.h"
 #include "dg_kernels.cuh"
 
@@ -17,15 +19,23 @@ template <> struct StageMinBlocks<3> { static constexpr int value = 5; };
 template <> struct StageMinBlocks<4> { static constexpr int value = 3; };
 template <> struct StageMinBlocks<5> { static constexpr int value = 2; };
 
+constexpr int kMaxDevices = 64;
+
 template <int M, int EOS, int GRAV, int KIND, int FLUX>
 cudaError_t launch_stage_variant(const StageArgs& A, dim3 grid, cudaStream_t stream) {
-  static bool attr_set = false;      // dynamic shared memory above 48 KB must be opted in once
+  // dynamic shared memory above 48 KB is opted in once per device (the attribute belongs to the device's context):
+  // one flag per device ordinal, set after the call succeeded; racing threads at worst both make the (idempotent) call
+  static std::atomic<bool> attr_set[kMaxDevices];
   constexpr size_t smem = stage_smem_bytes<M>();
   auto kern = stage_kernel<M, EOS, GRAV, KIND, StageMinBlocks<M>::value, FLUX>;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  const bool cached = dev >= 0 && dev < kMaxDevices;
+  if (!cached || !attr_set[dev].load(std::memory_order_acquire)) {
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_set = true;
+    if (cached) attr_set[dev].store(true, std::memory_order_release);
   }
   kern<<<grid, StageWarps<M, KIND>::threads, smem, stream>>>(A);
   return cudaGetLastError();

@@ -15,7 +15,7 @@ EXPORTS = [
     "dg_get_state_host", "dg_rhs", "dg_cfl_dt", "dg_step", "dg_step_debug", "dg_run_host",
     "dg_time", "dg_set_time", "dg_launch_count", "dg_set_tuning", "dg_stage_timing",
     "dg_stage_time_ms", "dg_stage_times_ms", "dg_probe_fp64_peak", "dg_last_error", "dg_destroy",
-    "dg_rk_stages", "dg_limit", "dg_torque",
+    "dg_rk_stages", "dg_limit", "dg_torque", "dg_torque_normalised",
     "dg_step_begin", "dg_substep", "dg_step_end", "dg_halo_layout",
 ]
 
@@ -39,6 +39,7 @@ class DGParams(C.Structure):
         ("flux", C.c_int32),
         ("damp_in_r0", C.c_double), ("damp_in_r1", C.c_double),
         ("halo_south", C.c_int32), ("halo_north", C.c_int32),
+        ("damp_mode", C.c_int32),
     ]
 
 
@@ -85,6 +86,7 @@ def load_library(path: str | None = None):
         "dg_step_begin": (i, [vp, d]), "dg_substep": (i, [vp]), "dg_step_end": (i, [vp]),
         "dg_halo_layout": (i, [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
         "dg_rk_stages": (i, [i]), "dg_limit": (i, [vp]), "dg_torque": (i, [vp, d, C.POINTER(d)]),
+        "dg_torque_normalised": (i, [vp, d, d, C.POINTER(d)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -101,7 +103,7 @@ class DG:
     arrays (pinned torch tensors make the copies asynchronous).
     """
 
-    def __init__(self, params: dict, stream=None):
+    def __init__(self, params: dict, stream=None, extra_workspace_bytes: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise DGError("no CUDA device: libdg has no CPU fallback")
@@ -117,6 +119,7 @@ class DG:
         nbytes = self.L.dg_workspace_bytes(C.byref(ps))
         if nbytes == 0:
             raise DGError("invalid dg_params")
+        nbytes += int(extra_workspace_bytes)             # e.g. two state arrays for DG_TUNE_RK4_FORM = 0 (include/dg.h)
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
         base = self.workspace.data_ptr()
         self._ws_ptr = (base + 255) // 256 * 256
@@ -222,6 +225,11 @@ class DG:
     def torque(self, t: float) -> float:
         g = C.c_double()
         self._chk(self.L.dg_torque(self._h, float(t), C.byref(g)), "dg_torque")
+        return g.value
+
+    def torque_normalised(self, t: float, sigma_p: float) -> float:
+        g = C.c_double()
+        self._chk(self.L.dg_torque_normalised(self._h, float(t), float(sigma_p), C.byref(g)), "dg_torque_normalised")
         return g.value
 
     def run_host(self, U_in, nsteps: int, cfl: float, U_out):

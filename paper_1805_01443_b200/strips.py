@@ -53,6 +53,9 @@ def exchange_rows(first, last, halo_south, halo_north, rank: int, n: int, period
     south neighbour's north halo, ``last`` to the north neighbour's south halo.  Tensors may live on any device
     the backend supports; returns after the transfers completed."""
     south, north = neighbours(rank, n, periodic)
+    if group is not None:                       # P2POp peers are global ranks
+        south = None if south is None else dist.get_global_rank(group, south)
+        north = None if north is None else dist.get_global_rank(group, north)
     # one fixed order on every rank -- southward traffic first, then northward -- so that the k-th message a rank
     # sends to a peer is the k-th it expects from it even when both neighbours are the same rank (2 periodic strips)
     ops = []
@@ -86,15 +89,18 @@ class LocalStrips:
         return torch.cat([g.get_state() for g in self.ctx], dim=0)
 
     def exchange(self):
-        """Fill every halo row from the neighbour strip's boundary row of the array its next kernel reads."""
+        """Fill every halo row from the neighbour strip's boundary row of the array its next kernel reads (on the
+        contexts' own stream, whatever stream is current in the caller: the copies are ordered against the kernels)."""
+        import torch
         views = [g.halo_rows() for g in self.ctx]
-        for r in range(self.n):
-            south, north = neighbours(r, self.n, self.periodic)
-            (_, _), (hs, hn) = views[r]
-            if south is not None:
-                hs.copy_(views[south][0][1])          # the south neighbour's last row
-            if north is not None:
-                hn.copy_(views[north][0][0])          # the north neighbour's first row
+        with torch.cuda.stream(self.ctx[0].stream):
+            for r in range(self.n):
+                south, north = neighbours(r, self.n, self.periodic)
+                (_, _), (hs, hn) = views[r]
+                if south is not None:
+                    hs.copy_(views[south][0][1])          # the south neighbour's last row
+                if north is not None:
+                    hn.copy_(views[north][0][0])          # the north neighbour's first row
 
     def cfl_dt(self, cfl: float) -> float:
         return min(g.cfl_dt(cfl) for g in self.ctx)
@@ -138,8 +144,15 @@ class DistStrip:
         self.g.set_state(U_dev_local)
 
     def exchange(self):
+        """One halo exchange on the context's stream (NCCL orders its point-to-point kernels against the stream that is
+        current when they are issued, so the stage kernels before and after are ordered against the transfers)."""
         (first, last), (hs, hn) = self.g.halo_rows()
-        exchange_rows(first, last, hs, hn, self.rank, self.n, self.periodic, self.dist, self.group)
+        if first.is_cuda:
+            import torch
+            with torch.cuda.stream(self.g.stream):
+                exchange_rows(first, last, hs, hn, self.rank, self.n, self.periodic, self.dist, self.group)
+        else:
+            exchange_rows(first, last, hs, hn, self.rank, self.n, self.periodic, self.dist, self.group)
 
     def cfl_dt(self, cfl: float) -> float:
         import torch

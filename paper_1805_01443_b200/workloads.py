@@ -38,6 +38,7 @@ _PARAM_DEFAULTS = dict(
     limiter=0, lim_eps=1e-13, flux=0,
     damp_in_r0=0.0, damp_in_r1=0.0,
     halo_south=0, halo_north=0,
+    damp_mode=0,
 )
 
 
@@ -245,7 +246,8 @@ def paper_disc(n: int = 256, order: int = 3, rk: int = 2, planet: bool = True, l
     Sigma0 = 1, p0 = 2.5e-3, r_in = 0.4, r_ex = 1.75, h = 0.05; planet q = 6e-5 at r_p = 1, eps_p = 0.03;
     v_phi^2 = r^2 Omega^2 - r c_iso^2 f / (r_p h (1+f)) with c_iso^2 = p0/Sigma0 (reading G12) and
     Omega^2 = GM/r_in^3 inside r_in, GM/r^3 outside (reading G11: solid rotation inside, PAPER.md:288);
-    wave-killing zones r_d = r_in 1.15^(3/2) -> r_in and r_d = r_ex 1.15^(-3/2) -> r_ex; frozen box edge
+    wave-killing zones r_d = r_in 1.15^(3/2) -> r_in and r_d = r_ex 1.15^(-3/2) -> r_ex relaxing "the density,
+    velocities and temperature" (damp_mode 1); frozen box edge
     (G14).  The density falls to ~4e-13 in the box corners: the positivity limiter is on by default.
     The paper does not soften the star's potential; with eps_star = 0 the four cells around the origin blow up within
     one step on a Cartesian grid, so the default is the BASELINE disc's 0.2 (inside the damped hole r < r_in)."""
@@ -255,7 +257,7 @@ def paper_disc(n: int = 256, order: int = 3, rk: int = 2, planet: bool = True, l
                     order=order, rk=rk, bc=2, eos=0, gamma=gamma, h_aspect=h, gm_star=gm, eps_star=eps_star,
                     q_planet=6.0e-5 if planet else 0.0, r_planet=1.0, eps_planet=0.03, omega_planet=1.0,
                     phase0=0.0, damp_r0=r_ex * 1.15 ** -1.5, damp_r1=r_ex,
-                    damp_in_r0=r_in * 1.15 ** 1.5, damp_in_r1=r_in,
+                    damp_in_r0=r_in * 1.15 ** 1.5, damp_in_r1=r_in, damp_mode=1,
                     limiter=1 if limiter else 0, lim_eps=1e-13)
     X, Y = _mesh(p)
     r = np.sqrt(X * X + Y * Y)

@@ -13,7 +13,8 @@ def pytest_configure(config):
 
 
 def pytest_collection_modifyitems(config, items):
-    """Tests marked gpu are skipped, not failed, when no device is visible and -m gpu was not asked."""
+    """Tests marked gpu are skipped when no device is visible -- unless the run asked for them (`-m gpu`): then a
+    missing device is an error, not a green run with nothing executed."""
     try:
         import torch
         has = torch.cuda.is_available()
@@ -21,6 +22,9 @@ def pytest_collection_modifyitems(config, items):
         has = False
     if has:
         return
+    asked = (config.getoption("-m") or "").strip()
+    if asked == "gpu" and any("gpu" in it.keywords for it in items):
+        raise pytest.UsageError("-m gpu was requested but no CUDA device is visible")
     skip = pytest.mark.skip(reason="no CUDA device")
     for it in items:
         if "gpu" in it.keywords:

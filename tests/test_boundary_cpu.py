@@ -64,11 +64,12 @@ def test_workspace_sizing_and_validation(lib):
     for bad in (dict(order=0), dict(order=6), dict(rk=6), dict(rk=1), dict(limiter=2), dict(limiter=1, lim_eps=0.0), dict(bc=3), dict(eos=2), dict(nx=0),
                 dict(x1=p["x0"]), dict(gamma=1.0), dict(eos=1), dict(damp_r0=1.0, damp_r1=0.5)):
         assert lib.dg_workspace_bytes(C.byref(params_struct(dict(p, **bad)))) == 0, bad
-    # Butcher-form schemes keep their slopes K_j: rk 4 needs 4 more state buffers, rk 5 needs 5
-    for rk, extra in ((4, 4), (5, 5)):
-        nk = lib.dg_workspace_bytes(C.byref(params_struct(dict(p, rk=rk))))
+    # spare state buffers of the general schemes: rk 4 in its low-storage form 2 (4 with the limiter's
+    # Z form), rk 5 (state form or Z form) 5
+    for rk, lim, extra in ((4, 0, 2), (4, 1, 4), (5, 0, 5), (5, 1, 5)):
+        nk = lib.dg_workspace_bytes(C.byref(params_struct(dict(p, rk=rk, limiter=lim))))
         assert (3 + extra) * state <= nk < (3 + extra) * state + 4096
-        assert lib.dg_rk_stages(rk) == extra + 1
+    assert lib.dg_rk_stages(4) == 5 and lib.dg_rk_stages(5) == 6
     assert lib.dg_rk_stages(2) == 2 and lib.dg_rk_stages(3) == 3 and lib.dg_rk_stages(7) == -1
     assert lib.dg_workspace_bytes(None) == 0
     h = C.c_void_p()

@@ -345,9 +345,11 @@ def test_limiter_parity(DG, case):
 def test_limited_step_parity(DG, case, rk):
     """A full step with the limiter after every sub-step, from a state the limiter has
     just made admissible but which the step drives negative again in places; fused tail
-    (limiter + wave-killing + CFL in one pass) against the debug path and the oracle."""
+    (limiter + wave-killing + CFL in one pass) against the debug path and the oracle, at north_star's 1e-12.
+    lim_eps = 1e-2 here: the floor sets the conditioning of the step that follows (reading L6; the
+    production floor 1e-13 is covered by test_limited_step_parity_production_floor)."""
     p, U = _make(case, rk=rk, seed=7)
-    U, hit = _negative_spots(U, seed=70, frac=0.1, lo=0.2, hi=0.8)
+    U, hit = _negative_spots(U, seed=70, frac=0.1)
     p = dict(p, limiter=1, lim_eps=1e-2)
     if case["eos"] == 1:
         p["damp_r0"], p["damp_r1"] = 0.6, 1.2
@@ -365,15 +367,44 @@ def test_limited_step_parity(DG, case, rk):
     st = g.step_debug(dt).cpu().numpy()
     for s in range(st.shape[0]):
         assert np.isfinite(st_ref[s]).all()
-        assert rel_err(st[s], st_ref[s]) < 2 * TOL_STAGE, f"sub-step {s + 1}"
-    assert rel_err(g.get_state().cpu().numpy(), ref.get_state()) < 2 * TOL_STAGE
+        assert rel_err(st[s], st_ref[s]) < TOL_STAGE, f"sub-step {s + 1}"
+    assert rel_err(g.get_state().cpu().numpy(), ref.get_state()) < TOL_STAGE
     g2 = DG(p)
     g2.set_state(dev(U1))
     g2.step(dt)
-    assert rel_err(g2.get_state().cpu().numpy(), ref.get_state()) < 2 * TOL_STAGE
-    # the seeded spots leave cells whose average density is ~1e-3 of the maximum: v = m / rho_bar there
-    # amplifies the 1e-12-of-max state difference, so the fused reduction is compared at 1e-9
+    assert rel_err(g2.get_state().cpu().numpy(), ref.get_state()) < TOL_STAGE
+    # v = m / rho_bar in the CFL reduction: cells with rho_bar ~ 1e-2 of the maximum amplify the 1e-12-of-max state
+    # difference by 1e2, and the maximum picks the worst cell (reading L6)
     assert abs(g2.cfl_dt(0.2) / ref.cfl_dt(0.2) - 1.0) < 1e-9
+
+
+@pytest.mark.parametrize("rk", [3, 5])
+@pytest.mark.parametrize("case", [c for c in NEXT_CASES[:5] if c["eos"] == 0], ids=_id)
+def test_limited_step_parity_production_floor(DG, case, rk):
+    """The same with the production floor lim_eps = 1e-13 (Zhang & Shu's value) on the ideal-gas cases.  A limited
+    point's density is then rho = 1e-13 +- ulp(rho_bar)/2, i.e. known to 1e-3 RELATIVE on both sides, and the step
+    that follows divides by it (v = m/rho): the two implementations cannot agree on that step better than that
+    conditioning allows.  Measured on B200: 7e-11 .. 4e-10 per sub-step (reading L6); asserted 2e-9.
+    (The isothermal cases are not run at this floor: nothing bounds m/rho there and the ORACLE goes non-finite.)"""
+    p, U = _make(case, rk=rk, seed=7)
+    U, hit = _negative_spots(U, seed=70, frac=0.1)
+    p = dict(p, limiter=1, lim_eps=1e-13)
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    ref.limit()
+    U1 = ref.get_state()
+    ref.set_state(U1)
+    g = DG(p)
+    g.set_state(dev(U))
+    g.limit()
+    assert rel_err(g.get_state().cpu().numpy(), U1) < TOL_STAGE     # the limiter itself: 1e-12
+    g.set_state(dev(U1))
+    dt = 0.5 * ref.cfl_dt(0.2)
+    st_ref = ref.step_debug(dt)
+    st = g.step_debug(dt).cpu().numpy()
+    assert np.isfinite(st_ref).all()
+    for s in range(st.shape[0]):
+        assert rel_err(st[s], st_ref[s]) < 2e-9, f"sub-step {s + 1}"
 
 
 @pytest.mark.parametrize("case", NEXT_CASES[1:4], ids=_id)
@@ -639,7 +670,7 @@ def test_rk4_low_storage_form_equals_the_butcher_form(DG):
         ref.step(dt)
         outs = []
         for form in (1, 0):
-            g = DG(p)
+            g = DG(p, extra_workspace_bytes=2 * U.nbytes * 2)   # form 0 needs two more state arrays (include/dg.h)
             g.set_tuning(4, form)
             g.set_state(dev(U))
             g.step(dt)
@@ -695,3 +726,201 @@ def test_dist_strip_single_rank_nccl(DG):
         assert s.torque(g.time) == g.torque(g.time)
     finally:
         dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------------
+# Round 2: BASELINE.json's literal disc constants, damp_mode 1, Gresho with its own boundary, guards
+def test_literal_baseline_disc_rhs_and_step_parity_full_size(DG):
+    """BASELINE.json configs[3] AS WRITTEN (floor 1e-6, star softening 0.02; taper 0.05 per SURVEY.md 8(d)) at 1024^2,
+    order 5: dg_rhs and every stage of one SSP-RK3 step against the oracle on every element (the unlimited scheme is
+    finite for the first steps; bench.py's `literal_with_limiter` block times this workload with limiter = 1)."""
+    p, U = W.disc(1024, 5, planet=True, noise=1e-4, **W.LITERAL_BASELINE_DISC)
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    g = DG(p)
+    g.set_state(dev(U))
+    dt = ref.cfl_dt(0.2)
+    assert abs(g.cfl_dt(0.2) / dt - 1.0) < 1e-13
+    L = g.rhs(0.0).cpu().numpy()
+    Lref = ref.rhs(0.0)
+    assert np.isfinite(Lref).all()
+    assert rhs_effect_err(L, Lref, U, dt) < TOL_STAGE
+    del L, Lref
+    st_ref = ref.step_debug(dt)
+    st = g.step_debug(dt).cpu().numpy()
+    for s in range(3):
+        assert rel_err(st[s], st_ref[s]) < TOL_STAGE, f"stage {s + 1}"
+
+
+def test_literal_baseline_disc_free_running(DG):
+    """configs[1]/[3]'s literal constants at 128^2: free-running steps for as long as the unlimited ORACLE keeps every
+    nodal density positive (at most 100), within 1e-10; then 100 steps with limiter = 1 (order 3 and 5)."""
+    for m in (3, 5):
+        p, U = W.disc(128, m, planet=True, noise=1e-4, **W.LITERAL_BASELINE_DISC)
+        ref = oracle.RefDG(p, omp=True)
+        ref.set_state(U)
+        g = DG(p)
+        g.set_state(dev(U))
+        done = 0
+        for _ in range(100):
+            dt = ref.cfl_dt(0.2)
+            ref.step(dt)
+            S = ref.get_state()
+            if not (np.isfinite(S).all() and W.evaluate_nodal(p, S)[:, :, 0].min() > 0):
+                break
+            g.step(dt)
+            done += 1
+        assert done >= 10, done
+        # compare at the last step both took
+        ref2 = oracle.RefDG(p, omp=True)
+        ref2.set_state(U)
+        g2 = DG(p)
+        g2.set_state(dev(U))
+        for _ in range(done):
+            dt = ref2.cfl_dt(0.2)
+            assert abs(g2.cfl_dt(0.2) / dt - 1.0) < 1e-9
+            ref2.step(dt)
+            g2.step(dt)
+        assert rel_err(g2.get_state().cpu().numpy(), ref2.get_state()) < TOL_100, (m, done)
+        pl = dict(p, limiter=1)
+        assert _run_100(DG, pl, U) < TOL_100
+
+
+@pytest.mark.parametrize("lim", [0, 1])
+@pytest.mark.parametrize("rk", [3, 5])
+def test_primitive_wave_killing_parity(DG, rk, lim):
+    """damp_mode 1 (density, velocities, temperature): the limiter's last pass (limiter on), the
+    stand-alone kernel after the last stage (limiter off) and the debug path against the oracle, both zones."""
+    p, U = W.random_smooth(70, 33, 4, seed=12, eos=0, bc=2, rk=rk, gravity=True)
+    p.update(damp_r0=0.9, damp_r1=1.2, damp_in_r0=0.4, damp_in_r1=0.3, damp_mode=1, limiter=lim)
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    dt = ref.cfl_dt(0.2)
+    ref.step(dt)
+    ref0 = oracle.RefDG(dict(p, damp_mode=0), omp=True)
+    ref0.set_state(U)
+    ref0.step(dt)
+    assert rel_err(ref0.get_state(), ref.get_state()) > 1e-9          # the two modes are different operations
+    for debug in (False, True):
+        g = DG(p)
+        g.set_tuning(1, 5)
+        g.set_state(dev(U))
+        g.step_debug(dt) if debug else g.step(dt)
+        assert rel_err(g.get_state().cpu().numpy(), ref.get_state()) < TOL_STAGE
+        assert abs(g.cfl_dt(0.2) / ref.cfl_dt(0.2) - 1.0) < 1e-12
+
+
+def test_paper_disc_uses_primitive_wave_killing_and_normalised_torque(DG):
+    """NEXT-3 as the row is written: the paper's disc relaxes density, velocities and temperature in both zones
+    (PAPER.md:313), and the torque is quoted as gamma Gamma / Gamma_0."""
+    p, U = W.paper_disc(48, 3, rk=2)
+    assert p["damp_mode"] == 1
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    ref.limit()
+    U1 = ref.get_state()
+    ref.set_state(U1)
+    g = DG(p)
+    g.set_state(dev(U1))
+    for _ in range(20):
+        dt = ref.cfl_dt(0.2)
+        ref.step(dt)
+        g.step(dt)
+    assert rel_err(g.get_state().cpu().numpy(), ref.get_state()) < TOL_100
+    t = ref.time
+    a, b = g.torque_normalised(t, 1.0), ref.torque_normalised(t, 1.0)
+    assert abs(a - b) < 1e-9 * max(1.0, abs(b))
+    assert abs(a - p["gamma"] * g.torque(t) / (1.0 * 1.0 * 1.0 * p["q_planet"] / p["h_aspect"] ** 2)) < 1e-12 * max(1.0, abs(a))
+
+
+@pytest.mark.parametrize("m", [2, 3, 4])
+def test_gresho_gradient_free_boundary_parity(DG, m):
+    """The Gresho vortex with the paper's own "gradient free" boundaries (bc 1): dg_rhs, every stage
+    of a step, and 100 free-running steps against the oracle.  (The Table 1 SOFT PIN is compared on a periodic
+    box, reading B1; parity needs no such choice.)"""
+    p, U = W.gresho(40, m, rk=min(m, 3))
+    assert p["bc"] == 1
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    g = DG(p)
+    g.set_state(dev(U))
+    dt = ref.cfl_dt(0.2)
+    assert rhs_effect_err(g.rhs(0.0).cpu().numpy(), ref.rhs(0.0), U, dt) < TOL_STAGE
+    st_ref = ref.step_debug(dt)
+    st = g.step_debug(dt).cpu().numpy()
+    for s in range(st.shape[0]):
+        assert rel_err(st[s], st_ref[s]) < TOL_STAGE
+    assert _run_100(DG, p, U) < TOL_100
+
+
+def test_calls_refused_inside_a_split_step(DG):
+    """Between dg_step_begin and dg_step_end the spare buffers hold live sub-step data (include/dg.h): every call
+    that would use them as scratch, or act on a state that is not a time level, returns DG_ESTATE, and the step
+    still completes bitwise like an undivided one."""
+    from paper_1805_01443_b200 import dg as B
+    p, U = W.disc(64, 3, planet=True, noise=1e-4)
+    g = DG(p)
+    g.set_state(dev(U))
+    g.step_begin(1e-3)
+    g.substep()
+    out = g.new_device_state()
+    hout = torch.empty(U.shape, dtype=torch.float64).pin_memory()
+    for call in (lambda: g.rhs(0.0), lambda: g.get_state(out), lambda: g.get_state_host(hout), lambda: g.limit(),
+                 lambda: g.cfl_dt(0.2), lambda: g.torque(0.0), lambda: g.step_debug(1e-3), lambda: g.step(1e-3)):
+        with pytest.raises(B.DGError, match=r"\(-3\)"):
+            call()
+    g.substep()
+    g.substep()
+    g.step_end()
+    g2 = DG(p)
+    g2.set_state(dev(U))
+    g2.step(1e-3)
+    assert torch.equal(g.get_state(), g2.get_state())
+
+
+def _dist_strip_worker(rank, size, port, q):
+    import os
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    torch.cuda.set_device(rank)
+    dist.init_process_group("nccl", rank=rank, world_size=size, device_id=torch.device("cuda", rank))
+    from paper_1805_01443_b200 import DG as _DG, strips
+    p, U = W.disc(64, 3, planet=True, noise=1e-4, half_width=2.0)
+    s = strips.DistStrip(_DG, p)
+    s.set_state(dev(U[s.j0:s.j1]))
+    for _ in range(3):
+        s.step(s.cfl_dt(0.2))
+    q.put((rank, s.j0, s.j1, s.g.get_state().cpu().numpy(), s.time))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_dist_strip_two_gpus_bitwise(DG):
+    """`strips.DistStrip` with one rank per GPU (NCCL point-to-point halo exchange): two strips on two GPUs
+    reproduce the undivided domain bitwise.  Needs two visible GPUs (none of this pool's runs has them)."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs 2 GPUs")
+    import socket
+    import torch.multiprocessing as mp
+    s_ = socket.socket()
+    s_.bind(("127.0.0.1", 0))
+    port = s_.getsockname()[1]
+    s_.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_dist_strip_worker, args=(r, 2, port, q)) for r in range(2)]
+    for pr in procs:
+        pr.start()
+    parts = sorted(q.get(timeout=300) for _ in procs)
+    for pr in procs:
+        pr.join(timeout=60)
+        assert pr.exitcode == 0
+    p, U = W.disc(64, 3, planet=True, noise=1e-4, half_width=2.0)
+    g = DG(p)
+    g.set_state(dev(U))
+    for _ in range(3):
+        g.step(g.cfl_dt(0.2))
+    whole = g.get_state().cpu().numpy()
+    for _rank, j0, j1, part, t in parts:
+        np.testing.assert_array_equal(part, whole[j0:j1])
+        assert t == g.time
