@@ -5,6 +5,7 @@
     python bench.py --impl reference [--steps K] [--warmup W]     # the CPU oracle, as it stands
     python bench.py --sweep                                       # configs[4]: orders x grids table
     python bench.py --variants                                    # RK(5,4), Cash-Karp, limiter, torque
+    torchrun ... bench.py --gpus N --decomp strips                # ONE problem cut into N strips (strong scaling; NEXT-4)
 
 A *step* is one full time step of the hot path on BASELINE configs[3] (planet-disc, 1024^2 cells,
 order 5, SSP-RK3): dg_cfl_dt (row a10 of SURVEY.md 8(a); its reduction rides on the previous last
@@ -42,16 +43,33 @@ FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md, used onl
 
 
 # ------------------------------------------------------------------------------------------------
-def workload_config(n: int, order: int) -> dict:
+DISC_RECIPE = dict(floor=1e-2, taper=0.1, eps_star=0.2)      # workloads.disc defaults
+
+
+def workload_config(n: int, order: int, replicas: int = 1, literal: bool = False, limiter: int = 0,
+                    parallelism: str = "replicas") -> dict:
+    """`config` of the JSON line: the workload as it is actually run, including where its disc constants deviate
+    from BASELINE.json's text.  The reference arm prints the same dict for the grid it really ran."""
+    from paper_1805_01443_b200 import workloads as W
+    rec = dict(W.LITERAL_BASELINE_DISC) if literal else dict(DISC_RECIPE)
     state = n * n * 4 * order * order * 8
+    dev = ("disc constants as BASELINE.json writes them (floor 1e-6, star softening 0.02; taper 0.05 per SURVEY.md 8(d))"
+           if literal else
+           f"DEVIATES from BASELINE.json configs[3] (floor 1e-6, star softening 0.02): runs floor {rec['floor']:g}, "
+           f"tanh taper {rec['taper']:g}, star softening {rec['eps_star']:g}, because north_star's step list has no limiter "
+           f"and the literal constants go negative without one: see DESIGN.md section 3; the literal constants with "
+           f"limiter = 1 are timed in the `literal_with_limiter` block of this line")
     return {
-        "workload": f"BASELINE configs[3]: planet-disc (locally isothermal h=0.05, q=1e-5 planet, frozen bc, "
+        "workload": f"BASELINE configs[3] shape: planet-disc (locally isothermal h=0.05, q=1e-5 planet, frozen bc, "
                     f"wave-killing zone r>2.2, seeded 1e-4 noise), {n}x{n} cells, DG order {order} "
-                    f"({order * order} modes x 4 vars per cell), SSP-RK3, CFL {CFL}, dt recomputed every step",
+                    f"({order * order} modes x 4 vars per cell), SSP-RK3, CFL {CFL}, dt recomputed every step, "
+                    f"limiter {'on' if limiter else 'off'}; {dev}",
         "nx": n, "ny": n, "order": order, "rk": 3, "state_bytes": state,
+        "disc_floor": rec["floor"], "disc_taper": rec["taper"], "star_softening": rec["eps_star"], "limiter": limiter,
+        "deviates_from_baseline": not literal,
         "l2": "inputs larger than L2: each stage reads >= one %.0f MB state array (L2 is 126 MB); no flush" % (state / 1e6)
         if state > 2 * 126e6 else "state fits L2 and is NOT flushed between steps: L2-assisted number",
-        "parallelism": "replicas",
+        "parallelism": parallelism, "replicas": replicas,
     }
 
 
@@ -165,7 +183,160 @@ def stage_bytes_per_launch(p: dict) -> tuple[float, dict]:
                         "per_dof_update": round(per_launch / (nx * ny * m * m), 2)}
 
 
-MODEL_FLOPS = {1: 441, 2: 1668, 3: 4017, 4: 7824, 5: 13425}   # modal sum-factorised model, per cell-stage
+def load_exec_counts(order: int, n: int):
+    """Executed fp64 thread instructions per stage launch from the committed ncu capture
+    (profiles/stage_exec_counts.csv: sm__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum per kernel of
+    one step), averaged over the step's launches: (dfma, dmul, dadd) or None."""
+    path = os.path.join(ROOT, "profiles", "stage_exec_counts.csv")
+    try:
+        with open(path) as f:
+            rows = [ln.strip().split(";") for ln in f if ln.strip() and not ln.startswith("#")]
+        hdr, rows = rows[0], rows[1:]
+        idx = {k: i for i, k in enumerate(hdr)}
+        sel = [r for r in rows if int(r[idx["order"]]) == order and int(r[idx["n"]]) == n]
+        if not sel:
+            return None
+        return tuple(sum(float(r[idx[k]]) for r in sel) / len(sel) for k in ("dfma", "dmul", "dadd"))
+    except Exception:
+        return None
+
+
+
+
+def fp64_block(m: int, n: int, stage_ms: float, fp64_peak) -> dict:
+    """EXECUTED fp64 work of the stage kernel (instruction counts of the committed ncu capture, FMA = 2 flops) over
+    the live CUDA-event time, against the DFMA peak measured on this GPU.  No model flops: the collocation kernel does
+    not execute SURVEY.md 8(a)'s modal operation count."""
+    ex = load_exec_counts(m, n)
+    out = {"peak_tflops": fp64_peak, "peak_source": "dg_probe_fp64_peak: register-resident DFMA loop on this GPU",
+           "executed_thread_inst_per_launch": None, "executed_flops_per_cell_stage": None,
+           "achieved_executed_tflops": None, "frac_executed": None,
+           "source": "profiles/stage_exec_counts.csv (ncu sm__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum)"}
+    if ex and stage_ms > 0:
+        dfma, dmul, dadd = ex
+        flops = 2.0 * dfma + dmul + dadd
+        out.update({"executed_thread_inst_per_launch": {"dfma": dfma, "dmul": dmul, "dadd": dadd},
+                    "executed_flops_per_cell_stage": flops / (n * n),
+                    "achieved_executed_tflops": flops / (stage_ms * 1e-3) / 1e12,
+                    "frac_executed": (flops / (stage_ms * 1e-3) / 1e12 / fp64_peak) if fp64_peak else None,
+                    "pipe_slots_frac": ((dfma + dmul + dadd) / (stage_ms * 1e-3) / 1e12 / (fp64_peak / 2.0))
+                    if fp64_peak else None})
+    return out
+
+
+def literal_block(args, dev, peak) -> dict:
+    """BASELINE.json configs[3] with its LITERAL disc constants (floor 1e-6, star softening 0.02) and the paper's
+    positivity limiter after every sub-step (limiter = 1): same grid, same order, own timing."""
+    import numpy as np
+    import torch
+    from paper_1805_01443_b200 import DG, workloads as W
+    n, m = args.n, args.order
+    p, U = W.disc(n, m, planet=True, noise=1e-4, **W.LITERAL_BASELINE_DISC)
+    p = dict(p, limiter=1)
+    g = DG(p)
+    g.set_state(torch.from_numpy(U).to(dev))
+    del U
+    g.limit()
+    for _ in range(3):
+        g.step(g.cfl_dt(CFL))
+    torch.cuda.synchronize()
+    steps = max(1, min(args.steps, 50))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    g.stage_timing(True)
+    l0 = g.launch_count
+    e0.record()
+    for _ in range(steps):
+        g.step(g.cfl_dt(CFL))
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    stage_ms, _ = g.stage_time_ms()
+    g.stage_timing(False)
+    launches = (g.launch_count - l0) / steps
+    S = g.get_state().cpu().numpy()
+    ok = bool(np.isfinite(S).all() and (W.evaluate_nodal(p, S)[:, :, 0] > 0).all())
+    _, acct = stage_bytes_per_launch(p)
+    arrays = step_arrays(p, acct["damping_zone_fraction"])
+    gbs = arrays * acct["state_bytes"] / (ms * 1e-3) / 1e9
+    g.close()
+    return {"config": workload_config(n, m, literal=True, limiter=1), "steps": steps, "ms_per_step": ms,
+            "value": W.dof_count(p) * p["rk"] / (ms * 1e-3), "unit": UNIT, "stage_kernel_ms": stage_ms,
+            "launches_per_step": launches, "state_valid": ok,
+            "roofline": {"bound": "hbm", "kernels": "3 x stage_kernel + 3 x limit_kernel (the last carries wave-killing + CFL)",
+                         "algorithmic_arrays_per_step": round(arrays, 3), "achieved": gbs, "peak": peak, "unit": "GB/s",
+                         "frac": gbs / peak}}
+
+
+def run_strips_arm(args) -> dict | None:
+    """--decomp strips: ONE problem (the bench workload) cut into N strips of whole cell rows, one rank per GPU
+    (strips.DistStrip: NCCL point-to-point halo exchange per sub-step on a side stream, overlapped with the interior
+    row segments; all_reduce(MIN) for dt).  Strong scaling.  SURVEY.md 8(e)/(f) NEXT-4; unmeasured on more than one
+    GPU in this pool."""
+    import socket
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1805_01443_b200 import DG, replicas, strips, workloads as W
+    from paper_1805_01443_b200.build import build
+
+    rank, local, size = replicas.world()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if not replicas.init("nccl", dev):                       # a single rank still goes through the same code path
+        if os.environ.get("TORCHELASTIC_RUN_ID") and os.environ.get("MASTER_PORT"):
+            # under torchrun the store is the agent's (a tcp:// rendezvous would wait for a server that never starts)
+            dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
+        else:
+            s_ = socket.socket()
+            s_.bind(("127.0.0.1", 0))
+            port = s_.getsockname()[1]
+            s_.close()
+            dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1, device_id=dev)
+    if rank == 0:
+        build()
+    dist.barrier()
+    n, m = args.n, args.order
+    p, U = W.disc(n, m, planet=True, noise=1e-4)
+    s = strips.DistStrip(DG, p)
+    s.set_state(torch.from_numpy(np.ascontiguousarray(U[s.j0:s.j1])).to(dev))
+    del U
+    for _ in range(max(args.warmup, 3)):
+        s.step(s.cfl_dt(CFL))
+    torch.cuda.synchronize()
+    sampler = ClockSampler(visible_index(local))
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = s.g.launch_count
+    dist.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    ev0.record()
+    for _ in range(args.steps):
+        s.step(s.cfl_dt(CFL))
+    ev1.record()
+    torch.cuda.synchronize()
+    dist.barrier()
+    clocks = sampler.stop()
+    launches = s.g.launch_count - l0
+    rows = s.j1 - s.j0
+    value, t_ms = replicas.throughput(ev0.elapsed_time(ev1), rows * n * m * m * p["rk"] * args.steps, dev)
+    row_bytes = ((n + 31) // 32) * 32 * 4 * m * m * 8
+    out = None
+    if rank == 0:
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": size, "steps": args.steps,
+               "warmup": max(args.warmup, 3), "ms_per_step": t_ms / args.steps, "higher_is_better": True,
+               "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+               "config": workload_config(n, m, replicas=1, parallelism="strips"),
+               "gpu_launches": int(launches), "clocks": clocks,
+               "decomposition": {"strips": size, "rows_per_strip": rows, "exchange": "one row per neighbour per sub-step, "
+                                 "NCCL send/recv on a side stream, overlapped with the interior row segments",
+                                 "halo_bytes_per_neighbour_per_substep": row_bytes, "substeps_per_step": p["rk"],
+                                 "collectives_per_step": "1 all_reduce(MIN) of one double (dt)"},
+               "note": "multi-GPU scaling of this mode is unmeasured in this pool (one GPU per run)"}
+    dist.barrier()
+    dist.destroy_process_group()
+    return out
 
 
 def run_cuda_arm(args) -> dict | None:
@@ -282,12 +453,11 @@ def run_cuda_arm(args) -> dict | None:
     peak, peak_src = load_peaks()
     bpl, acct = stage_bytes_per_launch(p)
     achieved = bpl / (stage_ms * 1e-3) / 1e9 if stage_ms > 0 else 0.0
-    flops = MODEL_FLOPS.get(m, 0) * n * n
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": size, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": t_ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": dict(workload_config(n, m), replicas=size),
+        "config": workload_config(n, m, replicas=size),
         "cell_stage_updates_per_s": value / (m * m),
         "state_valid": ok,
         "gpu_launches": int(launches),
@@ -300,12 +470,7 @@ def run_cuda_arm(args) -> dict | None:
             "accounting": acct, "frac_of_nominal_8TBs": achieved / 8000.0,
             "stage_share_of_step": stage_ms * rk / (t_ms / args.steps) if t_ms > 0 else None,
         },
-        "fp64": {
-            "peak_tflops": fp64_peak, "peak_source": "dg_probe_fp64_peak: register-resident DFMA loop on this GPU",
-            "model_flops_per_cell_stage": MODEL_FLOPS.get(m), "model": "SURVEY.md 8(a) modal sum-factorised count",
-            "achieved_model_tflops": flops / (stage_ms * 1e-3) / 1e12 if stage_ms > 0 else None,
-            "frac_model": (flops / (stage_ms * 1e-3) / 1e12 / fp64_peak) if stage_ms > 0 and fp64_peak else None,
-        },
+        "fp64": fp64_block(m, n, stage_ms, fp64_peak),
         "e2e": {
             "value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes,
             "steps": ke, "ms_per_step": e2e_s * 1e3 / ke,
@@ -316,6 +481,9 @@ def run_cuda_arm(args) -> dict | None:
                                       "one step's H2D overlaps the other's D2H; every step pays both copies"},
         },
     }
+    if size == 1 and not args.no_literal:
+        torch.cuda.empty_cache()
+        out["literal_with_limiter"] = literal_block(args, dev, peak)
     if size == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(m, budget_s=args.cpu_budget)
     replicas.finish()
@@ -373,13 +541,14 @@ def run_reference_arm(args) -> dict | None:
         if cand * cand * m * m * 3 * total / r0 <= budget:
             n = cand
     rate, dt, threads = _oracle_rate(n, m, args.steps, warm=args.warmup)
-    sample = (f"each step = one SSP-RK3 step of the same planet-disc recipe at {n}x{n} cells (order {m}); "
-              f"oracle/ref_dg.cpp as it stands, OpenMP over cell rows")
+    sample = (f"each step = one SSP-RK3 step of the same planet-disc recipe at {n}x{n} cells (order {m})"
+              + ("" if n == args.n else f", a bounded sample of the {args.n}x{args.n} workload sized for the time budget")
+              + "; oracle/ref_dg.cpp as it stands, OpenMP over cell rows")
     return {
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(args.n, m),
+        "config": workload_config(n, m, replicas=args.gpus),     # the grid the oracle really ran (n <= --n)
         "cpu_baseline": {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -525,6 +694,10 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-literal", action="store_true", help="skip the literal_with_limiter block")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "strips"],
+                    help="N > 1: independent replicas (default, north_star) or ONE problem cut into N strips along y "
+                         "with a halo exchange per sub-step (strips.DistStrip; strong scaling)")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--variants", action="store_true")
     ap.add_argument("--sweep-grids", default="256,512,1024,2048")
@@ -537,7 +710,12 @@ def main():
     if args.variants:
         run_variants(args)
         return
-    out = run_reference_arm(args) if args.impl == "reference" else run_cuda_arm(args)
+    if args.impl == "reference":
+        out = run_reference_arm(args)
+    elif args.decomp == "strips":
+        out = run_strips_arm(args)
+    else:
+        out = run_cuda_arm(args)
     if out is not None:
         print(json.dumps(out), flush=True)
 

@@ -122,6 +122,11 @@ int dg_step(dg_ctx*, double dt);
 int dg_step_begin(dg_ctx*, double dt);
 int dg_substep(dg_ctx*);
 int dg_step_end(dg_ctx*);
+/* A sub-step in two launches, so that the halo exchange overlaps the bulk of the strip: part 0 = the row segments
+ * that touch no halo row (launch it while the exchange is in flight), part 1 = the first and last row segment
+ * (after the halo rows have arrived), followed by the limiter pass when it is on.  dg_substep = part 0 + part 1.
+ * Same arithmetic, same result bitwise.  DG_ESTATE if called out of order. */
+int dg_substep_part(dg_ctx*, int part);
 /* Between dg_step_begin and dg_step_end the workspace's spare state buffers hold live sub-step data: dg_rhs,
  * dg_get_state*, dg_limit, dg_cfl_dt, dg_torque*, dg_step and dg_step_debug return DG_ESTATE there (they use those
  * buffers as scratch, or would act on a state that is not a time level).  dg_set_state* abandons the split step. */

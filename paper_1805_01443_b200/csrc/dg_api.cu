@@ -115,6 +115,7 @@ struct dg_ctx {
   int rk4_low_storage;        // 1: Table 1's scheme in its Shu-Osher form (default), 0: Butcher form
   Ssp54 ssp54;
   bool step_active;           // between dg_step_begin and dg_step_end
+  bool step_part_done;        // the interior part of the next sub-step has been launched (dg_substep_part)
   int step_next;              // next sub-step of the split step
   double step_dt;
   int step_A;
@@ -216,8 +217,13 @@ struct GenArgs {               // K_GEN / K_GENL: out = a u^n + b u + sum_j kc[j
   double* zout = nullptr;
 };
 
+// which row segments of the grid a launch covers: all of them, or -- for a strip of a decomposed domain whose
+// halo rows are still in flight -- the interior ones first and the first / last one afterwards
+enum { PART_ALL = -1, PART_INTERIOR = 0, PART_EDGES = 1 };
+constexpr int EDGE_ROWS = 4;
+
 int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout, double a, double b,
-                 double dt, double t, int kind, const GenArgs* ga = nullptr, double nfac = -1.0) {
+                 double dt, double t, int kind, const GenArgs* ga = nullptr, double nfac = -1.0, int part = PART_ALL) {
   // nfac >= 0: the factor of dt N in the output when it is not b (low-storage RK(5,4))
   StageArgs A{};
   const bool gen = kind == K_GEN || kind == K_GENL;
@@ -241,7 +247,23 @@ int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout,
     for (int k = 0; k < c->L.m; ++k) { A.T.Dx[q][k] *= beta; A.T.Dy[q][k] *= beta; }
   }
   const int grav = c->p.gm_star > 0.0 ? (c->p.q_planet > 0.0 ? G_PLANET : G_STAR) : G_NONE;
-  dim3 grid(c->L.nbx, (c->p.ny + A.rows - 1) / A.rows);
+  // rows next to a halo row wait for the exchange: a few rows only (EDGE_ROWS), so that the second launch is short
+  const int ny = c->p.ny;
+  const int edge = std::min(EDGE_ROWS, ny / 2);
+  auto blocks = [&](int r0, int r1) { return r1 > r0 ? (r1 - r0 + A.rows - 1) / A.rows : 0; };
+  A.rowA0 = 0; A.rowA1 = ny; A.rowB0 = A.rowB1 = 0;
+  if (part == PART_INTERIOR) {
+    if (edge == 0) return DG_OK;                  // a one-row strip is all edge
+    A.rowA0 = edge; A.rowA1 = ny - edge;
+  }
+  else if (part == PART_EDGES) {
+    if (edge > 0) { A.rows = std::min(A.rows, edge); A.rowA1 = edge; A.rowB0 = ny - edge; A.rowB1 = ny; }
+    // (edge = 0: a one-row strip is all edge, region A = everything)
+  }
+  A.nblkA = blocks(A.rowA0, A.rowA1);
+  const int count = A.nblkA + blocks(A.rowB0, A.rowB1);
+  if (count <= 0) return DG_OK;
+  dim3 grid(c->L.nbx, count);
   const bool timed = c->timing && c->ev_used + 2 <= c->evs.size();
   if (timed) cudaEventRecord(c->evs[c->ev_used], c->stream);
   cudaError_t e;
@@ -329,6 +351,7 @@ int finish_set_state(dg_ctx* c) {
   c->has_state = true;
   c->wmax_valid = false;
   c->step_active = false;   // a new state abandons a split step in progress
+  c->step_part_done = false;
   c->t = c->p.t0;
   return DG_OK;
 }
@@ -454,7 +477,7 @@ int step_begin(dg_ctx* c, const StepPlan& P) {
 }
 
 // Sub-step i: one fused stage kernel, then the limiter when it is on, then (debug) the copy-out.
-int run_substep(dg_ctx* c, const StepPlan& P, int i) {
+int run_substep(dg_ctx* c, const StepPlan& P, int i, int part = PART_ALL) {
   const double dt = P.dt;
   const bool last = i + 1 == P.k;
   const double* qin = substep_in_ptr(c, P, i);
@@ -470,11 +493,11 @@ int run_substep(dg_ctx* c, const StepPlan& P, int i) {
     const double ts = c->t + bt.c[i] * dt;
     const int B = (P.A + 1) % 3, Cc = (P.A + 2) % 3;
     if (i == 0) {
-      e = launch_stage(c, qin, qn, qout, 0.0, 1.0, dt, ts, K_FIRST, nullptr, S.beta[0]);
+      e = launch_stage(c, qin, qn, qout, 0.0, 1.0, dt, ts, K_FIRST, nullptr, S.beta[0], part);
     } else if (i < 3) {
-      e = launch_stage(c, qin, qn, qout, 1.0 - S.alpha[i], S.alpha[i], dt, ts, K_MID, nullptr, S.beta[i]);
+      e = launch_stage(c, qin, qn, qout, 1.0 - S.alpha[i], S.alpha[i], dt, ts, K_MID, nullptr, S.beta[i], part);
     } else if (i == 3) {
-      e = launch_stage(c, qin, qn, qout, 1.0 - S.alpha[3], S.alpha[3], dt, ts, K_MID, nullptr, S.beta[3]);
+      e = launch_stage(c, qin, qn, qout, 1.0 - S.alpha[3], S.alpha[3], dt, ts, K_MID, nullptr, S.beta[3], part);
     } else {
       // u^{n+1} = c2 y_3 + c3 y_4 + c4 y_5 + d3 dt L(y_4) + d4 dt L(y_5), with dt L(y_4) eliminated through
       // y_5 = (1 - alpha_4) u^n + alpha_4 y_4 + beta_4 dt L(y_4): no slope is ever stored
@@ -484,15 +507,15 @@ int run_substep(dg_ctx* c, const StepPlan& P, int i) {
       ga.kin[0] = c->q(Cc); ga.kc[0] = S.c2;
       ga.kin[1] = c->q(B); ga.kc[1] = S.c3 - r * S.alpha[3];
       const int kind = (P.fuse_tail && !P.lim) ? K_GENL : K_GEN;
-      e = launch_stage(c, qin, qn, qout, -r * (1.0 - S.alpha[3]), S.c4 + r, dt, ts, kind, &ga, S.d4);
+      e = launch_stage(c, qin, qn, qout, -r * (1.0 - S.alpha[3]), S.c4 + r, dt, ts, kind, &ga, S.d4, part);
     }
   } else if (c->p.rk <= 3) {
     // SSP-RK in Shu-Osher form, stage times c = (0,1) / (0,1,1/2)
     const int last_kind = (P.fuse_tail && !P.lim) ? (P.damp ? K_LASTD : K_LAST) : K_MID;
-    if (i == 0)                  e = launch_stage(c, qin, qn, qout, 0.0, 1.0, dt, c->t, K_FIRST);
-    else if (c->p.rk == 2)       e = launch_stage(c, qin, qn, qout, 0.5, 0.5, dt, c->t + dt, last_kind);
-    else if (i == 1)             e = launch_stage(c, qin, qn, qout, 0.75, 0.25, dt, c->t + dt, K_MID);
-    else                         e = launch_stage(c, qin, qn, qout, 1.0 / 3.0, 2.0 / 3.0, dt, c->t + 0.5 * dt, last_kind);
+    if (i == 0)                  e = launch_stage(c, qin, qn, qout, 0.0, 1.0, dt, c->t, K_FIRST, nullptr, -1.0, part);
+    else if (c->p.rk == 2)       e = launch_stage(c, qin, qn, qout, 0.5, 0.5, dt, c->t + dt, last_kind, nullptr, -1.0, part);
+    else if (i == 1)             e = launch_stage(c, qin, qn, qout, 0.75, 0.25, dt, c->t + dt, K_MID, nullptr, -1.0, part);
+    else                         e = launch_stage(c, qin, qn, qout, 1.0 / 3.0, 2.0 / 3.0, dt, c->t + 0.5 * dt, last_kind, nullptr, -1.0, part);
   } else {
     // General explicit scheme (Appendix A) in state form (dg_tables.h): sub-step i reads its
     // input y_{i+1} (with halo), u^n and the earlier states with a non-zero coefficient, and writes y_{i+2}.
@@ -508,10 +531,10 @@ int run_substep(dg_ctx* c, const StepPlan& P, int i) {
       for (int j = 0; j < i; ++j)
         if (Z.z[i][j] != 0.0) { ga.kin[ga.nk] = c->kbuf(j); ga.kc[ga.nk] = Z.z[i][j]; ga.nk++; }
       ga.zout = last ? nullptr : c->kbuf(i);
-      e = launch_stage(c, qin, qn, qout, Z.abar[i], 0.0, dt, ts, K_GEN, &ga, Z.beta[i]);
+      e = launch_stage(c, qin, qn, qout, Z.abar[i], 0.0, dt, ts, K_GEN, &ga, Z.beta[i], part);
     } else if (i == 0) {
       const StateForm F = state_form_from_butcher(bt);
-      e = launch_stage(c, qin, qn, qout, 0.0, 1.0, dt, ts, K_FIRST, nullptr, F.beta[0]);
+      e = launch_stage(c, qin, qn, qout, 0.0, 1.0, dt, ts, K_FIRST, nullptr, F.beta[0], part);
     } else {
       const StateForm F = state_form_from_butcher(bt);
       GenArgs ga{};
@@ -519,10 +542,11 @@ int run_substep(dg_ctx* c, const StepPlan& P, int i) {
         if (F.g[i][m] != 0.0) { ga.kin[ga.nk] = c->kbuf(m - 1); ga.kc[ga.nk] = F.g[i][m]; ga.nk++; }
       int kind = (last && P.fuse_tail) ? K_GENL : K_GEN;
       if (ga.nk == 0) kind = kind == K_GEN ? K_MID : (P.damp ? K_LASTD : K_LAST);   // nothing to gather: the plain SSP stage
-      e = launch_stage(c, qin, qn, qout, F.g[i][0], F.g[i][i], dt, ts, kind, &ga, F.beta[i]);
+      e = launch_stage(c, qin, qn, qout, F.g[i][0], F.g[i][i], dt, ts, kind, &ga, F.beta[i], part);
     }
   }
   if (e) return e;
+  if (part == PART_INTERIOR) return DG_OK;        // the limiter and the copy-out follow the edge segments
   if (P.lim && (e = launch_limit(c, qout, last && P.fuse_tail, dt))) return e;
   if (P.stages) {
     const size_t n = (size_t)c->p.ny * c->p.nx * 4 * c->L.m * c->L.m;
@@ -615,6 +639,7 @@ int dg_init(const dg_params* p, void* workspace, size_t ws_bytes, void* cuda_str
     }
   }
   c->step_active = false;
+  c->step_part_done = false;
   c->step_next = 0;
   c->gen_pf = 3;
   c->launches = 0;
@@ -791,6 +816,7 @@ int dg_step_begin(dg_ctx* c, double dt) {
   int e = step_begin(c, P);
   if (e) return e;
   c->step_active = true;
+  c->step_part_done = false;
   c->step_next = 0;
   c->step_dt = dt;
   c->step_A = P.A;
@@ -803,9 +829,26 @@ int dg_substep(dg_ctx* c) {
   StepPlan P = make_plan(c, c->step_dt, nullptr);
   P.A = c->step_A;
   if (c->step_next >= P.k) return fail(c, DG_ESTATE, "dg_substep: all sub-steps of this step have run");
+  if (c->step_part_done) return fail(c, DG_ESTATE, "dg_substep: finish the sub-step with dg_substep_part(1)");
   int e = run_substep(c, P, c->step_next);
   if (!e) c->step_next++;
   return e;
+}
+
+int dg_substep_part(dg_ctx* c, int part) {
+  if (!c) return DG_EINVAL;
+  if (!c->step_active) return fail(c, DG_ESTATE, "dg_substep_part: no split step in progress");
+  if (part != PART_INTERIOR && part != PART_EDGES) return fail(c, DG_EINVAL, "dg_substep_part: part must be 0 or 1");
+  StepPlan P = make_plan(c, c->step_dt, nullptr);
+  P.A = c->step_A;
+  if (c->step_next >= P.k) return fail(c, DG_ESTATE, "dg_substep_part: all sub-steps of this step have run");
+  if (part == PART_INTERIOR && c->step_part_done) return fail(c, DG_ESTATE, "dg_substep_part: interior already launched");
+  if (part == PART_EDGES && !c->step_part_done) return fail(c, DG_ESTATE, "dg_substep_part: launch the interior (part 0) first");
+  int e = run_substep(c, P, c->step_next, part);
+  if (e) return e;
+  if (part == PART_INTERIOR) c->step_part_done = true;
+  else { c->step_part_done = false; c->step_next++; }
+  return DG_OK;
 }
 
 int dg_step_end(dg_ctx* c) {

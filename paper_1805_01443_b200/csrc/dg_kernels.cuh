@@ -114,6 +114,10 @@ struct StageArgs {
   double a, b, dt;            // out = a u^n + b u^(s-1) + beta N; beta = b dt is folded into T and ph
   DampArgs D;
   int rows;
+  // rows a launch covers: thread blocks y < nblkA march over [rowA0, rowA1) in segments of `rows` rows, the others
+  // over [rowB0, rowB1).  A whole-domain launch is region A = [0, ny); a strip of a decomposed domain launches its
+  // interior rows while the halo exchange is in flight and the few rows next to the halos afterwards.
+  int rowA0, rowA1, nblkA, rowB0, rowB1;
   // K_GEN / K_GENL: the earlier stage states the sub-step combines (besides u^n and its input) and their
   // coefficients
   const double* kin[MAXK];
@@ -407,8 +411,9 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   const DevTables& T = A.T;
   const bool valid = i < g.nx;
   const int last_lane = min(31, g.nx - 1 - ib * 32);
-  const int j0 = blockIdx.y * A.rows;
-  const int j1 = min(g.ny, j0 + A.rows);
+  const bool regA = (int)blockIdx.y < A.nblkA;
+  const int j0 = regA ? A.rowA0 + (int)blockIdx.y * A.rows : A.rowB0 + ((int)blockIdx.y - A.nblkA) * A.rows;
+  const int j1 = min(regA ? A.rowA1 : A.rowB1, j0 + A.rows);
   const size_t row_stride = (size_t)g.nbx * BS;
 
   const double xc = g.x0 + (i + 0.5) * g.dx;

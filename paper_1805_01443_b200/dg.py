@@ -16,7 +16,7 @@ EXPORTS = [
     "dg_time", "dg_set_time", "dg_launch_count", "dg_set_tuning", "dg_stage_timing",
     "dg_stage_time_ms", "dg_stage_times_ms", "dg_probe_fp64_peak", "dg_last_error", "dg_destroy",
     "dg_rk_stages", "dg_limit", "dg_torque", "dg_torque_normalised",
-    "dg_step_begin", "dg_substep", "dg_step_end", "dg_halo_layout",
+    "dg_step_begin", "dg_substep", "dg_substep_part", "dg_step_end", "dg_halo_layout",
 ]
 
 
@@ -83,7 +83,7 @@ def load_library(path: str | None = None):
         "dg_probe_fp64_peak": (i, [vp, C.POINTER(d)]),
         "dg_last_error": (C.c_char_p, [vp]),
         "dg_destroy": (None, [vp]),
-        "dg_step_begin": (i, [vp, d]), "dg_substep": (i, [vp]), "dg_step_end": (i, [vp]),
+        "dg_step_begin": (i, [vp, d]), "dg_substep": (i, [vp]), "dg_substep_part": (i, [vp, i]), "dg_step_end": (i, [vp]),
         "dg_halo_layout": (i, [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
         "dg_rk_stages": (i, [i]), "dg_limit": (i, [vp]), "dg_torque": (i, [vp, d, C.POINTER(d)]),
         "dg_torque_normalised": (i, [vp, d, d, C.POINTER(d)]),
@@ -196,6 +196,9 @@ class DG:
 
     def substep(self):
         self._chk(self.L.dg_substep(self._h), "dg_substep")
+
+    def substep_part(self, part: int):
+        self._chk(self.L.dg_substep_part(self._h, int(part)), "dg_substep_part")
 
     def step_end(self):
         self._chk(self.L.dg_step_end(self._h), "dg_step_end")

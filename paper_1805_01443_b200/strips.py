@@ -70,8 +70,35 @@ def exchange_rows(first, last, halo_south, halo_north, rank: int, n: int, period
         req.wait()
 
 
+class _Overlap:
+    """Stream plumbing shared by both strip drivers: the halo exchange of a sub-step runs on a side stream, ordered
+    after everything the compute stream has done so far, while the compute stream launches the interior row
+    segments (`dg_substep_part(0)`); the edge segments (`dg_substep_part(1)`) wait for the exchange."""
+
+    def __init__(self, compute_stream):
+        import torch
+        self.torch = torch
+        self.compute = compute_stream
+        self.comm = torch.cuda.Stream(device=compute_stream.device) if compute_stream is not None else None
+
+    def run(self, exchange, interior, edges):
+        if self.comm is None:                    # host tensors (the gloo test of the exchange logic): no streams
+            exchange()
+            interior()
+            edges()
+            return
+        torch = self.torch
+        self.comm.wait_stream(self.compute)      # the rows to send were written by earlier kernels of the compute stream
+        with torch.cuda.stream(self.comm):
+            exchange()
+        with torch.cuda.stream(self.compute):
+            interior()
+            self.compute.wait_stream(self.comm)  # halo rows have arrived
+            edges()
+
+
 class LocalStrips:
-    """All strips of a decomposed domain as separate contexts on the current device (one stream)."""
+    """All strips of a decomposed domain as separate contexts on the current device (one compute stream)."""
 
     def __init__(self, DG, params: dict, n: int):
         self.p = dict(params)
@@ -79,6 +106,7 @@ class LocalStrips:
         self.rows = split_rows(params["ny"], n)
         self.periodic = params["bc"] == 0
         self.ctx = [DG(strip_params(params, j0, j1, r, n)) for r, (j0, j1) in enumerate(self.rows)]
+        self.ov = _Overlap(self.ctx[0].stream)
 
     def set_state(self, U_dev):
         for g, (j0, j1) in zip(self.ctx, self.rows):
@@ -89,18 +117,16 @@ class LocalStrips:
         return torch.cat([g.get_state() for g in self.ctx], dim=0)
 
     def exchange(self):
-        """Fill every halo row from the neighbour strip's boundary row of the array its next kernel reads (on the
-        contexts' own stream, whatever stream is current in the caller: the copies are ordered against the kernels)."""
-        import torch
+        """Fill every halo row from the neighbour strip's boundary row of the array its next kernel reads (device
+        copies on whatever stream is current: `step` and `rhs` order them against the kernels)."""
         views = [g.halo_rows() for g in self.ctx]
-        with torch.cuda.stream(self.ctx[0].stream):
-            for r in range(self.n):
-                south, north = neighbours(r, self.n, self.periodic)
-                (_, _), (hs, hn) = views[r]
-                if south is not None:
-                    hs.copy_(views[south][0][1])          # the south neighbour's last row
-                if north is not None:
-                    hn.copy_(views[north][0][0])          # the north neighbour's first row
+        for r in range(self.n):
+            south, north = neighbours(r, self.n, self.periodic)
+            (_, _), (hs, hn) = views[r]
+            if south is not None:
+                hs.copy_(views[south][0][1])          # the south neighbour's last row
+            if north is not None:
+                hn.copy_(views[north][0][0])          # the north neighbour's first row
 
     def cfl_dt(self, cfl: float) -> float:
         return min(g.cfl_dt(cfl) for g in self.ctx)
@@ -109,15 +135,16 @@ class LocalStrips:
         for g in self.ctx:
             g.step_begin(dt)
         for _ in range(self.ctx[0].rk_stages):
-            self.exchange()
-            for g in self.ctx:
-                g.substep()
+            self.ov.run(self.exchange,
+                        lambda: [g.substep_part(0) for g in self.ctx],
+                        lambda: [g.substep_part(1) for g in self.ctx])
         for g in self.ctx:
             g.step_end()
 
     def rhs(self, t: float):
         import torch
-        self.exchange()
+        with torch.cuda.stream(self.ctx[0].stream):
+            self.exchange()
         return torch.cat([g.rhs(t) for g in self.ctx], dim=0)
 
     def torque(self, t: float) -> float:
@@ -139,20 +166,16 @@ class DistStrip:
         self.rows = split_rows(params["ny"], self.n)
         self.j0, self.j1 = self.rows[self.rank]
         self.g = DG(strip_params(params, self.j0, self.j1, self.rank, self.n))
+        self.ov = _Overlap(self.g.stream)
 
     def set_state(self, U_dev_local):
         self.g.set_state(U_dev_local)
 
     def exchange(self):
-        """One halo exchange on the context's stream (NCCL orders its point-to-point kernels against the stream that is
-        current when they are issued, so the stage kernels before and after are ordered against the transfers)."""
+        """One halo exchange (NCCL point-to-point operations are ordered against the stream that is current when they
+        are issued: `step` issues them on the side stream)."""
         (first, last), (hs, hn) = self.g.halo_rows()
-        if first.is_cuda:
-            import torch
-            with torch.cuda.stream(self.g.stream):
-                exchange_rows(first, last, hs, hn, self.rank, self.n, self.periodic, self.dist, self.group)
-        else:
-            exchange_rows(first, last, hs, hn, self.rank, self.n, self.periodic, self.dist, self.group)
+        exchange_rows(first, last, hs, hn, self.rank, self.n, self.periodic, self.dist, self.group)
 
     def cfl_dt(self, cfl: float) -> float:
         import torch
@@ -163,8 +186,7 @@ class DistStrip:
     def step(self, dt: float):
         self.g.step_begin(dt)
         for _ in range(self.g.rk_stages):
-            self.exchange()
-            self.g.substep()
+            self.ov.run(self.exchange, lambda: self.g.substep_part(0), lambda: self.g.substep_part(1))
         self.g.step_end()
 
     def torque(self, t: float) -> float:

@@ -654,6 +654,28 @@ def test_split_step_api_errors(DG):
     g2.set_state(dev(U))
     g2.step(0.01)
     np.testing.assert_array_equal(g.get_state().cpu().numpy(), g2.get_state().cpu().numpy())
+    # a sub-step in two launches (interior row segments, then the edge segments): order is enforced, result bitwise
+    p3, U3 = W.disc(64, 3, planet=True, noise=1e-4)
+    a, b = DG(p3), DG(p3)
+    for g_ in (a, b):
+        g_.set_tuning(1, 4)                                 # 16 row segments
+        g_.set_state(dev(U3))
+    a.step_begin(1e-3)
+    with pytest.raises(B.DGError):
+        a.substep_part(1)                                   # interior first
+    a.substep_part(0)
+    with pytest.raises(B.DGError):
+        a.substep_part(0)
+    with pytest.raises(B.DGError):
+        a.substep()                                         # finish the started sub-step first
+    a.substep_part(1)
+    a.substep()
+    a.substep_part(0)
+    a.substep_part(1)
+    a.step_end()
+    b.step(1e-3)
+    assert torch.equal(a.get_state(), b.get_state())
+    assert a.cfl_dt(0.2) == b.cfl_dt(0.2)
 
 
 def test_rk4_low_storage_form_equals_the_butcher_form(DG):

@@ -75,3 +75,40 @@ def test_halo_exchange_between_ranks(n, periodic):
         exp_s = 10.0 * south + 2.0 if south is not None else -1.0
         exp_n = 10.0 * north + 1.0 if north is not None else -1.0
         assert res[r] == (exp_s, exp_n), (r, res[r])
+
+
+def _group_worker(rank, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=3)
+    try:
+        grp = dist.new_group([0, 2])                        # strips live on global ranks 0 and 2 (group ranks 0, 1)
+        if rank in (0, 2):
+            gr = dist.get_rank(grp)
+            first = torch.full((5,), 10.0 * gr + 1.0, dtype=torch.float64)
+            last = torch.full((5,), 10.0 * gr + 2.0, dtype=torch.float64)
+            hs = torch.full((5,), -1.0, dtype=torch.float64)
+            hn = torch.full((5,), -1.0, dtype=torch.float64)
+            strips.exchange_rows(first, last, hs, hn, gr, 2, False, dist, grp)
+            out[rank] = (float(hs[0]), float(hn[0]))
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_halo_exchange_in_a_sub_group_uses_global_ranks():
+    """P2POp peers are global ranks: a decomposition over a sub-group (global ranks 0 and 2 of 3) must translate its
+    group-local neighbour ranks."""
+    port = _free_port()
+    with mp.Manager() as mgr:
+        out = mgr.dict()
+        mp.spawn(_group_worker, args=(port, out), nprocs=3, join=True)
+        res = dict(out)
+    assert res[0] == (-1.0, 11.0) and res[2] == (2.0, -1.0), res
+
+
+def test_overlap_plumbing_order_on_host():
+    """Without a compute stream (host tensors) the three phases of a sub-step run in order: exchange, interior, edges."""
+    calls = []
+    strips._Overlap(None).run(lambda: calls.append("x"), lambda: calls.append("i"), lambda: calls.append("e"))
+    assert calls == ["x", "i", "e"]
