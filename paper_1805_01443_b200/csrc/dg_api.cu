@@ -112,6 +112,7 @@ struct dg_ctx {
   int rows_per_cta;
   int fused_cfl;
   int gen_pf;
+  int stage_impl;             // DG_TUNE_STAGE_IMPL
   int rk4_low_storage;        // 1: Table 1's scheme in its Shu-Osher form (default), 0: Butcher form
   Ssp54 ssp54;
   bool step_active;           // between dg_step_begin and dg_step_end
@@ -232,6 +233,7 @@ int launch_stage(dg_ctx* c, const double* qprev, const double* qn, double* qout,
     A.nk = ga->nk; A.zout = ga->zout; A.gen_pf = c->gen_pf;
     for (int k = 0; k < ga->nk; ++k) { A.kin[k] = ga->kin[k]; A.kc[k] = ga->kc[k]; }
   }
+  A.impl = c->stage_impl;
   A.qprev = qprev; A.qn = qn; A.qout = qout; A.q0 = c->q0();
   A.btrW = c->btrW(); A.btrE = c->btrE(); A.btrS = c->btrS(); A.btrN = c->btrN();
   A.haloS = c->haloS(); A.haloN = c->haloN();
@@ -642,6 +644,7 @@ int dg_init(const dg_params* p, void* workspace, size_t ws_bytes, void* cuda_str
   c->step_part_done = false;
   c->step_next = 0;
   c->gen_pf = 3;
+  c->stage_impl = 0;
   c->launches = 0;
   c->timing = false;
   c->ev_used = 0;
@@ -921,6 +924,10 @@ int dg_set_tuning(dg_ctx* c, int key, int value) {
         return DG_ENOSPC;
       }
       c->rk4_low_storage = value ? 1 : 0;
+      return DG_OK;
+    case DG_TUNE_STAGE_IMPL:
+      if (value < 0 || value > 2) return fail(c, DG_EINVAL, "stage implementation must be 0..2");
+      c->stage_impl = value;
       return DG_OK;
     case DG_TUNE_GEN_PREFETCH:
       if (value < 0 || value > 3) return fail(c, DG_EINVAL, "prefetch mode must be 0..3");

@@ -125,6 +125,7 @@ struct StageArgs {
   double* zout;               // if set: also store a u^n + b u + beta N, the value before the kin terms are added
                               // (limiter runs keep these instead of stage states: the limiter changes the states)
   int nk;
+  int impl;                   // host-side choice of the kernel: 0 default, 1 dg::stage_kernel, 2 dg::stage_kernel_fh (dg_stage_fh.cuh)
   int gen_pf;                 // L2 prefetch of the epilogue's inputs: 0 none, 1 row start, 2 a row ahead (evicted before use: 1.7x DRAM reads), 3 at the x/y phase boundary
   Geom g;
   Phys ph;
@@ -540,6 +541,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       fence_proxy_async();                       // the slots about to be refilled were read through the generic proxy
       if (more) tile_issue(t + 2);               // row j+2 -> the slot row j-1 has just left
       if (use_un && j > j0) un_issue(j);         // sN is free again
+      if (use_un && more) bulk_prefetch_l2(A.qn + (size_t)(j + 1) * row_stride + (size_t)ib * BS, TILE_BYTES);   // so that the next row's copy comes from L2
       if (do_damp && more) prefetch_q0(j + 1);
       if (gen && A.gen_pf == 2 && more) prefetch_gen(j + 1);
       if (gen && A.gen_pf == 1 && j > j0) prefetch_gen(j);

@@ -7,6 +7,7 @@
 
 #include "dg_tables.h"
 #include "dg_kernels.cuh"
+#include "dg_stage_fh.cuh"
 
 namespace dg {
 
@@ -19,10 +20,35 @@ template <> struct StageMinBlocks<3> { static constexpr int value = 5; };
 template <> struct StageMinBlocks<4> { static constexpr int value = 3; };
 template <> struct StageMinBlocks<5> { static constexpr int value = 2; };
 
+// Orders whose default stage kernel is the one with the face-helper warp (dg_stage_fh.cuh): the orders where M worker
+// warps of 168 registers leave the schedulers unevenly filled.  The other orders keep dg::stage_kernel.
+template <int M> struct StageFaceHelper { static constexpr bool value = M == 5; };
+
 constexpr int kMaxDevices = 64;
 
 template <int M, int EOS, int GRAV, int KIND, int FLUX>
+cudaError_t launch_stage_variant_fh(const StageArgs& A, dim3 grid, cudaStream_t stream) {
+  static std::atomic<bool> attr_set[kMaxDevices];
+  constexpr size_t smem = stage_fh_smem_bytes<M>();
+  auto kern = stage_kernel_fh<M, EOS, GRAV, KIND, StageMinBlocks<M>::value, FLUX>;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  const bool cached = dev >= 0 && dev < kMaxDevices;
+  if (!cached || !attr_set[dev].load(std::memory_order_acquire)) {
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    if (cached) attr_set[dev].store(true, std::memory_order_release);
+  }
+  kern<<<grid, (M + 1) * 32, smem, stream>>>(A);
+  return cudaGetLastError();
+}
+
+template <int M, int EOS, int GRAV, int KIND, int FLUX>
 cudaError_t launch_stage_variant(const StageArgs& A, dim3 grid, cudaStream_t stream) {
+  if constexpr (StageFaceHelper<M>::value) {
+    if (A.impl != 1) return launch_stage_variant_fh<M, EOS, GRAV, KIND, FLUX>(A, grid, stream);
+  }
   // dynamic shared memory above 48 KB is opted in once per device (the attribute belongs to the device's context):
   // one flag per device ordinal, set after the call succeeded; racing threads at worst both make the (idempotent) call
   static std::atomic<bool> attr_set[kMaxDevices];

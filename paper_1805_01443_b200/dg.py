@@ -9,6 +9,9 @@ _LIB_PATH = os.path.join(_HERE, "libdg.so")
 
 DG_TUNE_ROWS_PER_CTA = 1
 DG_TUNE_FUSED_CFL = 2
+DG_TUNE_GEN_PREFETCH = 3
+DG_TUNE_RK4_FORM = 4
+DG_TUNE_STAGE_IMPL = 5
 
 EXPORTS = [
     "dg_workspace_bytes", "dg_init", "dg_set_state", "dg_set_state_host", "dg_get_state",
