@@ -362,11 +362,16 @@ __device__ __forceinline__ void fence_proxy_async() {
 //   sAvg      partial cell averages of the row just written (fused CFL reduction, row a10)
 // ---------------------------------------------------------------------------------------------
 constexpr int NST = 3;
+// Depth of the tile ring per order.  Deeper rings for the low orders (8 slots at order 1, 5 at order 2, whose rows are
+// short and tiles small) were measured and changed nothing (1024^2 / 2048^2: order 1 0.33 / 0.42 of the copy
+// bandwidth either way, order 2 0.58 / 0.68 against 0.61 / 0.71): those orders are bound by the latency of one
+// warp's row, not by the prefetch distance.
+template <int M> struct StageRing { static constexpr int value = NST; };
 
 template <int M>
 constexpr size_t stage_smem_bytes() {
   // tiles + sN + sRi + sAvg + mbarriers
-  return ((size_t)(NST + 1) * 4 * M * M * 32 + (size_t)M * M * 32 + (size_t)4 * M * 32) * sizeof(double) + 64;
+  return ((size_t)(StageRing<M>::value + 1) * 4 * M * M * 32 + (size_t)M * M * 32 + (size_t)4 * M * 32) * sizeof(double) + 128;
 }
 
 // Warps per thread block: M workers, plus -- at M = 5, in the stages that carry the fused CFL reduction -- one helper
@@ -389,15 +394,16 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   constexpr bool use_un = KIND == K_MID || KIND == K_LAST || KIND == K_LASTD || gen;
   constexpr bool do_cfl = KIND == K_LAST || KIND == K_LASTD || KIND == K_GENL;
   constexpr bool do_damp = KIND == K_LASTD || KIND == K_GENL;    // K_GENL: only if the zone is enabled
+  constexpr int NS = StageRing<M>::value;        // slots of the tile ring
   constexpr int C = 4 * M * M;                   // doubles per cell
   constexpr int BS = C * 32;                     // doubles per 32-cell tile
   constexpr uint32_t TILE_BYTES = BS * sizeof(double);
   extern __shared__ __align__(128) double smem[];
   double* tiles = smem;
-  double* sN = tiles + NST * BS;
+  double* sN = tiles + NS * BS;
   double* sRi = sN + BS;                         // [r][q][lane]
   double* sAvg = sRi + M * M * 32;               // [v][q][lane]
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(sAvg + 4 * M * 32);   // [NST] tiles, [NST] u^n
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(sAvg + 4 * M * 32);   // [NS] tiles, [NS] u^n
 
   const int tid = threadIdx.x;
   const int lane = tid & 31;
@@ -444,21 +450,21 @@ stage_kernel(const __grid_constant__ StageArgs A) {
   auto tile_issue = [&](int t) {                 // thread 0 only
     const int jr = tile_row(t);
     if (jr != -1) {
-      uint64_t* bar = mbar + t % NST;
+      uint64_t* bar = mbar + t % NS;
       const double* src = jr >= 0 ? A.qprev + jr * row_stride : (jr == -2 ? A.haloS : A.haloN);
       mbar_expect_tx(bar, TILE_BYTES);
-      bulk_g2s(tiles + (t % NST) * BS, src + (size_t)ib * BS, TILE_BYTES, bar);
+      bulk_g2s(tiles + (t % NS) * BS, src + (size_t)ib * BS, TILE_BYTES, bar);
     }
   };
   // k-th copy into a slot completes mbarrier phase k; tile 0 is the only one that can be absent
   // and still be followed by later copies into its slot (non-periodic bottom row)
   const int skip0 = tile_row(0) == -1 ? 1 : 0;
   auto tile_wait = [&](int t) {
-    if (tile_row(t) != -1) mbar_wait(mbar + t % NST, (uint32_t)((t / NST - (t % NST == 0 ? skip0 : 0)) & 1));
+    if (tile_row(t) != -1) mbar_wait(mbar + t % NS, (uint32_t)((t / NS - (t % NS == 0 ? skip0 : 0)) & 1));
   };
   auto un_issue = [&](int j) {                   // thread 0 only; u^n tile of row j -> sN
-    mbar_expect_tx(mbar + NST, TILE_BYTES);
-    bulk_g2s(sN, A.qn + (size_t)j * row_stride + (size_t)ib * BS, TILE_BYTES, mbar + NST);
+    mbar_expect_tx(mbar + NS, TILE_BYTES);
+    bulk_g2s(sN, A.qn + (size_t)j * row_stride + (size_t)ib * BS, TILE_BYTES, mbar + NS);
   };
   // the last stage also reads the initial state where the wave-killing zone is active: pull that
   // tile into L2 ahead of its use (cheap test on the tile's farthest corner)
@@ -483,15 +489,21 @@ stage_kernel(const __grid_constant__ StageArgs A) {
 
   if (tid == ISSUER) {
 #pragma unroll
-    for (int s = 0; s <= NST; ++s) mbar_init(mbar + s, 1);
+    for (int s = 0; s <= NS; ++s) mbar_init(mbar + s, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
+  constexpr int PFD = NS - 2;                    // rows ahead at which the u^n tile is pulled into L2
   if (tid == ISSUER) {
-    tile_issue(0);
-    tile_issue(1);
-    tile_issue(2);
+#pragma unroll
+    for (int s = 0; s < NS; ++s)
+      if (s <= j1 - j0 + 1) tile_issue(s);       // tiles 0 .. rows + 1 are all a segment needs
     if (use_un) un_issue(j0);
+    if (use_un) {
+#pragma unroll
+      for (int d = 1; d < PFD; ++d)
+        if (j0 + d < j1) bulk_prefetch_l2(A.qn + (size_t)(j0 + d) * row_stride + (size_t)ib * BS, TILE_BYTES);
+    }
     if (do_damp) prefetch_q0(j0);
     if (gen && A.gen_pf) prefetch_gen(j0);
   }
@@ -539,14 +551,15 @@ stage_kernel(const __grid_constant__ StageArgs A) {
     const bool more = j + 1 < j1;
     if (tid == ISSUER) {
       fence_proxy_async();                       // the slots about to be refilled were read through the generic proxy
-      if (more) tile_issue(t + 2);               // row j+2 -> the slot row j-1 has just left
+      if (t - 1 + NS <= j1 - j0 + 1) tile_issue(t - 1 + NS);   // -> the slot row j-1 has just left (NS = 3: row j+2)
       if (use_un && j > j0) un_issue(j);         // sN is free again
-      if (use_un && more) bulk_prefetch_l2(A.qn + (size_t)(j + 1) * row_stride + (size_t)ib * BS, TILE_BYTES);   // so that the next row's copy comes from L2
+      if (use_un && j + PFD < j1)                // so that a later row's copy comes from L2
+        bulk_prefetch_l2(A.qn + (size_t)(j + PFD) * row_stride + (size_t)ib * BS, TILE_BYTES);
       if (do_damp && more) prefetch_q0(j + 1);
       if (gen && A.gen_pf == 2 && more) prefetch_gen(j + 1);
       if (gen && A.gen_pf == 1 && j > j0) prefetch_gen(j);
     }
-    const double* tu = tiles + (t % NST) * BS + lane;
+    const double* tu = tiles + (t % NS) * BS + lane;
     const double yc = g.y0 + (j + 0.5) * g.dy;
 
     // fused CFL wave speed of the row finished in the previous iteration (row a10)
@@ -682,7 +695,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
         riemann2<FLUX, EOS, 0>(UL, FL, lamL, UW, FWo, lamWo, HW);
       }
       // a u^n (landed in sN) + x-part of beta N
-      if (use_un) mbar_wait(mbar + NST, (uint32_t)((t - 1) & 1));
+      if (use_un) mbar_wait(mbar + NS, (uint32_t)((t - 1) & 1));
 #pragma unroll
       for (int v = 0; v < 4; ++v)
 #pragma unroll
@@ -779,7 +792,7 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       Wave<FLUX> aLam;
       if (tile_row(t + 1) != -1) {
         tile_wait(t + 1);
-        column_trace<M>(tiles + ((t + 1) % NST) * BS + lane, 32, q, T.Im, aU);
+        column_trace<M>(tiles + ((t + 1) % NS) * BS + lane, 32, q, T.Im, aU);
         face_flux<EOS, 1, FLUX>(A.ph, aU, cs2N, cN, aG, aLam);
       } else if (g.bc == 1) {
 #pragma unroll

@@ -392,7 +392,7 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
         bool damp = false;
         if (do_damp && (KIND != K_GENL || A.D.on))
           damp = damp_factors(A.D, sqrt_fast(fma(xc, xc, yc * yc) + 1e-300), f0, ft);   // + tiny: a centre at the origin
-        constexpr bool early_q0 = do_damp && M <= 4;
+        constexpr bool early_q0 = do_damp;
         double z0[4][M];
         if (early_q0) {
           const double* __restrict__ q0e = A.q0 + j * row_stride + (size_t)ib * BS + lane;
