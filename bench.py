@@ -73,6 +73,19 @@ def workload_config(n: int, order: int, replicas: int = 1, literal: bool = False
     }
 
 
+STAGE_IMPL = 0                  # --stage-impl: DG_TUNE_STAGE_IMPL for every context this run creates (0 = library default)
+
+
+def new_dg(p: dict, **kw):
+    """A DG context with this run's --stage-impl applied."""
+    from paper_1805_01443_b200 import DG
+    from paper_1805_01443_b200.dg import DG_TUNE_STAGE_IMPL
+    g = DG(p, **kw)
+    if STAGE_IMPL:
+        g.set_tuning(DG_TUNE_STAGE_IMPL, STAGE_IMPL)
+    return g
+
+
 def load_peaks() -> tuple[float, str]:
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -233,7 +246,7 @@ def literal_block(args, dev, peak) -> dict:
     n, m = args.n, args.order
     p, U = W.disc(n, m, planet=True, noise=1e-4, **W.LITERAL_BASELINE_DISC)
     p = dict(p, limiter=1)
-    g = DG(p)
+    g = new_dg(p)
     g.set_state(torch.from_numpy(U).to(dev))
     del U
     g.limit()
@@ -359,7 +372,7 @@ def run_cuda_arm(args) -> dict | None:
     p, U = W.disc(n, m, planet=True, noise=1e-4)
     dof = W.dof_count(p)
     rk = p["rk"]
-    g = DG(p)
+    g = new_dg(p)
     Ud = torch.from_numpy(U).to(dev)
     g.set_state(Ud)
     for _ in range(max(args.warmup, 3)):
@@ -415,7 +428,7 @@ def run_cuda_arm(args) -> dict | None:
         for _ in range(2):
             st = torch.cuda.Stream(device=dev)
             with torch.cuda.stream(st):
-                gi = DG(p, stream=st)
+                gi = new_dg(p, stream=st)
             ctxs.append((gi, torch.from_numpy(U).pin_memory(), torch.empty_like(hin).pin_memory()))
 
         def worker(gi, hi, ho, k):
@@ -463,7 +476,10 @@ def run_cuda_arm(args) -> dict | None:
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {
-            "bound": "hbm", "kernel": "dg::stage_kernel<M=%d> (fused RK stage: rows a1-a9, a11, a12 + a10 in the last)" % m,
+            "bound": "hbm", "kernel": ("dg::stage_kernel_fh<M=%d> (fused RK stage, M worker warps + a helper warp: rows a1-a9, a11, a12 + a10 in the last)"
+                                       if (m == 5 and STAGE_IMPL != 1) else
+                                       "dg::stage_kernel<M=%d> (fused RK stage: rows a1-a9, a11, a12 + a10 in the last)") % m,
+            "stage_impl": STAGE_IMPL,
             "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
             "traffic": load_ncu_traffic(m, n), "peak_source": peak_src,
             "ms_per_launch": stage_ms, "launches_timed": int(n_timed), "bytes_per_launch": bpl,
@@ -568,7 +584,7 @@ def run_sweep(args):
     for n in grids:
         for m in orders:
             p, U = W.disc(n, m, planet=True, noise=1e-4)
-            g = DG(p)
+            g = new_dg(p)
             g.set_state(torch.from_numpy(U).cuda())
             del U
             for _ in range(5):
@@ -588,11 +604,16 @@ def run_sweep(args):
             bpl, acct = stage_bytes_per_launch(p)
             dof = W.dof_count(p)
             ach = bpl / (stage_ms * 1e-3) / 1e9
+            fits_l2 = acct["state_bytes"] * 3 < 126e6
             print(json.dumps({
                 "n": n, "order": m, "steps": steps, "dof_updates_per_s": dof * 3 * steps / (ms * 1e-3),
                 "cell_stage_updates_per_s": n * n * 3 * steps / (ms * 1e-3), "ms_per_step": ms / steps,
-                "stage_ms": stage_ms, "hbm_gbs": ach, "hbm_frac": ach / peak,
-                "state_mb": acct["state_bytes"] / 1e6, "fits_l2": acct["state_bytes"] * 3 < 126e6,
+                "stage_ms": stage_ms, "algorithmic_gbs": ach,
+                # an HBM fraction only where the three arrays of a stage do not fit the 126 MB L2; below that the
+                # state stays L2-resident between stages and the figure is a rate of algorithmic bytes, not of DRAM
+                "hbm_frac": None if fits_l2 else ach / peak,
+                "algorithmic_gbs_over_hbm_peak": ach / peak,
+                "state_mb": acct["state_bytes"] / 1e6, "fits_l2": fits_l2,
             }), flush=True)
             g.close()
             del g
@@ -638,7 +659,7 @@ def run_variants(args):
                        ("rk5 + limiter", {"rk": 5, "limiter": 1}), ("ssp33, HLL flux (isothermal)", {"flux": 1})):
         p, U = W.disc(n, m, planet=True, noise=1e-4)
         p.update(over)
-        g = DG(p)
+        g = new_dg(p)
         g.set_state(torch.from_numpy(U).cuda())
         del U
         for _ in range(3):
@@ -698,12 +719,17 @@ def main():
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "strips"],
                     help="N > 1: independent replicas (default, north_star) or ONE problem cut into N strips along y "
                          "with a halo exchange per sub-step (strips.DistStrip; strong scaling)")
+    ap.add_argument("--stage-impl", type=int, default=0, choices=[0, 1, 2],
+                    help="DG_TUNE_STAGE_IMPL (include/dg.h): 0 = the library's default stage kernel per order, "
+                         "1 = dg::stage_kernel (M worker warps) at every order, 2 = the helper-warp kernel where it exists")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--variants", action="store_true")
     ap.add_argument("--sweep-grids", default="256,512,1024,2048")
     ap.add_argument("--sweep-orders", default="1,2,3,4,5")
     ap.add_argument("--sweep-steps", type=int, default=50)
     args = ap.parse_args()
+    global STAGE_IMPL
+    STAGE_IMPL = args.stage_impl
     if args.sweep:
         run_sweep(args)
         return

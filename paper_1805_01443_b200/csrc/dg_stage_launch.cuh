@@ -46,8 +46,10 @@ cudaError_t launch_stage_variant_fh(const StageArgs& A, dim3 grid, cudaStream_t 
 
 template <int M, int EOS, int GRAV, int KIND, int FLUX>
 cudaError_t launch_stage_variant(const StageArgs& A, dim3 grid, cudaStream_t stream) {
+  // (the sub-steps of the general schemes, K_GEN, gather up to five more arrays in the epilogue and run faster on the
+  // M-warp kernel: Cash-Karp with the limiter 6.7 ms per 1024^2 order-5 step against 8.2)
   if constexpr (StageFaceHelper<M>::value) {
-    if (A.impl != 1) return launch_stage_variant_fh<M, EOS, GRAV, KIND, FLUX>(A, grid, stream);
+    if (A.impl == 2 || (A.impl == 0 && KIND != K_GEN)) return launch_stage_variant_fh<M, EOS, GRAV, KIND, FLUX>(A, grid, stream);
   }
   // dynamic shared memory above 48 KB is opted in once per device (the attribute belongs to the device's context):
   // one flag per device ordinal, set after the call succeeded; racing threads at worst both make the (idempotent) call
