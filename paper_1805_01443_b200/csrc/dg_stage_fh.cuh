@@ -111,7 +111,8 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
   double* tiles = smem;
   double* sN = tiles + NS * BS;                  // u^n landing buffer -> a u^n + x-part of beta N -> (fused CFL) partial averages
   double* sRi = sN + BS;                         // [r][q][lane]: 1/sqrt(x^2+y^2+eps^2) at the row's volume nodes
-  double* sHS = sRi + M * M * 32;                // [v][q][lane]: S-face fluxes (x2) of the segment's first row (prologue)
+  double* sHS = sRi + M * M * 32;                // [v][q][lane]: S-face fluxes (x2) of the segment's first row (prologue); then
+                                                 // the N-face fluxes one worker evaluates for another (M = 5)
   double* sHX = sHS + 4 * M * 32;                // [row parity][r][side][v]: W flux of cell 0, E flux of the last cell
   uint64_t* mbar = reinterpret_cast<uint64_t*>(sHX + 2 * M * 8);   // [NS] tiles, u^n
 
@@ -292,6 +293,47 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
   }
   __syncthreads();                               // tile 0's slot may be overwritten
 
+  // N face of column qn of the row whose tile is tlo: the row's trace UNq at eta = +1 against the S trace of the row
+  // above (tile tlo + 1) or the boundary condition
+  auto n_face = [&](int tlo, int jrow, int qn, const double (&UNq)[4], double (&HNq)[4]) {
+    const double xqn = xc + g.hdx * T.xi[qn];
+    const double yN = g.y0 + (jrow + 1) * g.dy;
+    double cs2N = 0.0, cN = 0.0;
+    if (EOS == 1) {
+      cs2N = A.ph.h2gm * rsqrt_fast(fma(xqn, xqn, fma(yN, yN, A.ph.eps2s)));
+      cN = sqrt_fast(cs2N);
+    }
+    double GNo[4];
+    Wave<FLUX> lamNo;
+    face_flux<EOS, 1, FLUX>(A.ph, UNq, cs2N, cN, GNo, lamNo);
+    double aU[4], aG[4];
+    Wave<FLUX> aLam;
+    if (tile_row(tlo + 1) != -1) {
+      column_trace<M>(tiles + ((tlo + 1) % NS) * BS + lane, 32, qn, T.Im, aU);
+      face_flux<EOS, 1, FLUX>(A.ph, aU, cs2N, cN, aG, aLam);
+    } else if (g.bc == 1) {
+#pragma unroll
+      for (int v = 0; v < 4; ++v) { aU[v] = UNq[v]; aG[v] = GNo[v]; }
+      aLam = lamNo;
+    } else {
+#pragma unroll
+      for (int v = 0; v < 4; ++v) aU[v] = __ldg(A.btrN + ((size_t)(ib * 4 + v) * M + qn) * 32 + lane);
+      face_flux<EOS, 1, FLUX>(A.ph, aU, cs2N, cN, aG, aLam);
+    }
+    riemann2<FLUX, EOS, 1>(UNq, GNo, lamNo, aU, aG, aLam, HNq);
+  };
+  // Balance between the schedulers (M = 5).  Warp slots are handed out in order (two blocks of six: slots 0..5 and
+  // 6..11, scheduler = slot mod 4), so in both blocks workers 0, 2, 4 sit three to a scheduler and workers 1, 3 share
+  // theirs with one other worker and a helper that idles most of the row.  Workers 1 and 3 therefore also do the N
+  // face of columns 0 and M - 1 (first thing in their Y phase, through sHS) and workers 0 and M - 1 skip theirs:
+  // 3 x 0.85 against 2 x 1.15 + helper instead of 3 x 1 against 2 x 1 + helper.  Correct under any slot layout.
+  // Measured at 1024^2: first / middle stage 0.450 / 0.490 ms instead of 0.464 / 0.494; in the stages whose helper also
+  // carries the CFL reduction its scheduler has no room to spare (last stage 0.582 instead of 0.566), so not there.
+  constexpr bool REBAL = M == 5 && !do_cfl;
+  const bool donor = REBAL && (w == 0 || w == M - 1);
+  const bool taker = REBAL && (w == 1 || w == M - 2);
+  const int pair = w <= 1 ? 0 : 1;               // donor 0 <-> taker 1 (barrier 8), donor M-1 <-> taker M-2 (barrier 9)
+
   // Two loops over the rows, one per role, meeting at the same named barriers: what each role carries from row to
   // row (the workers' S-face flux, the helper's neighbour lines) costs registers in its own loop only.
   if (worker) {
@@ -379,6 +421,17 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
       bar_sync_named(2, NWORK);
 
       // =========================== Y phase: xi-column q = w ===========================
+      if (taker) {                               // the N face of a three-to-a-scheduler worker's column, for it
+        const int qx = pair == 0 ? 0 : M - 1;
+        bar_sync_named(3 + w, 64);               // the tile of the row above has landed
+        double UNx[4], HNx[4];
+        column_trace<M>(tu, 32, qx, T.Ip, UNx);
+        n_face(t, j, qx, UNx, HNx);
+#pragma unroll
+        for (int v = 0; v < 4; ++v) sHS[(v * M + qx) * 32 + lane] = HNx[v];
+        __threadfence_block();
+        bar_arrive_named(8 + pair, 64);
+      }
       {
         const int q = w;
         const double xq = xc + g.hdx * T.xi[q];
@@ -407,8 +460,10 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
           double u[4];
 #pragma unroll
           for (int v = 0; v < 4; ++v) u[v] = tu[((v * M + r) * M + q) * 32];
+          if (!donor) {
 #pragma unroll
-          for (int v = 0; v < 4; ++v) UN[v] = fma(T.Ip[r], u[v], UN[v]);
+            for (int v = 0; v < 4; ++v) UN[v] = fma(T.Ip[r], u[v], UN[v]);
+          }
           // gravity (row a3); the isothermal sound speed shares the star's 1/r_s
           double cs2 = 0.0, gx = 0.0, gy = 0.0;
           if (need_ri) {
@@ -445,33 +500,16 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
           }
         }
         // north face: own trace against the S trace of the row above (tile t+1: the helper arrives at barrier 3 + w
-        // once it has seen that tile land)
-        bar_sync_named(3 + w, 64);
-        const double yN = g.y0 + (j + 1) * g.dy;
-        double cs2N = 0.0, cN = 0.0;
-        if (EOS == 1) {
-          cs2N = A.ph.h2gm * rsqrt_fast(fma(xq, xq, fma(yN, yN, A.ph.eps2s)));
-          cN = sqrt_fast(cs2N);
-        }
-        double GNo[4];
-        Wave<FLUX> lamNo;
-        face_flux<EOS, 1, FLUX>(A.ph, UN, cs2N, cN, GNo, lamNo);
-        double aU[4], aG[4];
-        Wave<FLUX> aLam;
-        if (tile_row(t + 1) != -1) {
-          column_trace<M>(tiles + ((t + 1) % NS) * BS + lane, 32, q, T.Im, aU);
-          face_flux<EOS, 1, FLUX>(A.ph, aU, cs2N, cN, aG, aLam);
-        } else if (g.bc == 1) {
-#pragma unroll
-          for (int v = 0; v < 4; ++v) { aU[v] = UN[v]; aG[v] = GNo[v]; }
-          aLam = lamNo;
-        } else {
-#pragma unroll
-          for (int v = 0; v < 4; ++v) aU[v] = __ldg(A.btrN + ((size_t)(ib * 4 + v) * M + q) * 32 + lane);
-          face_flux<EOS, 1, FLUX>(A.ph, aU, cs2N, cN, aG, aLam);
-        }
+        // once it has seen that tile land), or -- workers 0 and M-1 at M = 5 -- what workers 1 and M-2 have put into sHS
         double HN[4];
-        riemann2<FLUX, EOS, 1>(UN, GNo, lamNo, aU, aG, aLam, HN);
+        if (donor) {
+          bar_sync_named(8 + pair, 64);
+#pragma unroll
+          for (int v = 0; v < 4; ++v) HN[v] = sHS[(v * M + q) * 32 + lane];
+        } else {
+          if (!taker) bar_sync_named(3 + w, 64);
+          n_face(t, j, q, UN, HN);
+        }
 
         // modal update in nodal form + RK combination (rows a8, a9) and store
         const size_t cell_off = j * row_stride + (size_t)ib * BS + lane;
@@ -553,7 +591,8 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
       }
       tile_wait(t + 1);                          // sent a whole row ago; the workers' N faces and the next row read it
 #pragma unroll
-      for (int k = 0; k < M; ++k) bar_arrive_named(3 + k, 64);
+      for (int k = 0; k < M; ++k)
+        if (!(REBAL && (k == 0 || k == M - 1))) bar_arrive_named(3 + k, 64);   // (those two take their N face from a neighbour)
       if (gen && A.gen_pf == 3 && issuer) prefetch_gen(j);
       // next row's outer x-faces (the neighbours' lines were requested a row ago), then the request for the row after
       if (more) edge_faces(j + 1, tiles + ((t + 1) % NS) * BS, sHX + ((j + 1 - j0) & 1) * (M * 8));
