@@ -189,8 +189,9 @@ long long dg_launch_count(const dg_ctx*);
                                    printed tableau's row ratios (default); 0 = the generic state form */
 #define DG_TUNE_STAGE_IMPL   5   /* which fused stage kernel runs: 0 = the default (order 5: the kernel with the helper warp,
                                    dg_stage_fh.cuh, except for the sub-steps of the general schemes that gather earlier
-                                   stage states; orders 1..4: M worker warps), 1 = M worker warps (dg::stage_kernel)
-                                   everywhere, 2 = the helper-warp kernel wherever it exists.  Same results to a few ulp. */
+                                   stage states; order 1: the register-only kernel, dg_stage_m1fv.cuh; orders 2..4: M
+                                   worker warps), 1 = M worker warps (dg::stage_kernel) at every order, 2 = like 0 but
+                                   the helper-warp kernel for every sub-step of order 5.  Same results to a few ulp. */
 int dg_set_tuning(dg_ctx*, int key, int value);
 
 /* Average-duration probe: enqueue CUDA events around the stage kernels of the next dg_step calls.

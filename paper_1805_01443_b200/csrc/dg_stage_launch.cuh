@@ -8,6 +8,7 @@
 #include "dg_tables.h"
 #include "dg_kernels.cuh"
 #include "dg_stage_fh.cuh"
+#include "dg_stage_m1fv.cuh"
 
 namespace dg {
 
@@ -46,6 +47,12 @@ cudaError_t launch_stage_variant_fh(const StageArgs& A, dim3 grid, cudaStream_t 
 
 template <int M, int EOS, int GRAV, int KIND, int FLUX>
 cudaError_t launch_stage_variant(const StageArgs& A, dim3 grid, cudaStream_t stream) {
+  if constexpr (M == 1) {                        // order 1: the register-only kernel (dg_stage_m1fv.cuh), one warp per segment of rows
+    if (A.impl != 1 && A.g.nx % 32 != 1) {
+      stage_kernel_m1<EOS, GRAV, KIND, FLUX><<<dim3(grid.x, (grid.y + M1_WARPS - 1) / M1_WARPS), M1_WARPS * 32, 0, stream>>>(A);
+      return cudaGetLastError();
+    }
+  }
   // (the sub-steps of the general schemes, K_GEN, gather up to five more arrays in the epilogue and run faster on the
   // M-warp kernel: Cash-Karp with the limiter 6.7 ms per 1024^2 order-5 step against 8.2)
   if constexpr (StageFaceHelper<M>::value) {
