@@ -13,8 +13,10 @@
 //       * the S face of the segment's first row (prologue);
 //       * TMA issue, mbarrier waits for the tiles, L2 prefetches, the fused CFL reduction.
 //
-// Measured at 1024^2, order 5 (B200): first / middle / last stage 0.464 / 0.494 / 0.566 ms against 0.469 / 0.487 /
-// 0.650 ms of dg::stage_kernel.  Variants that were built and measured slower (profiles/r02_fh_variants.md): the helper
+// Why a sixth warp is free: five warps of 168 registers make two blocks per SM = 10 warps; 12 x 168 x 32 registers still
+// fit the register file (3 warps per scheduler), and the shared memory of a block does not grow (114.6 KB).
+// Measured at 1024^2, order 5 (B200): first / middle / last stage 0.450 / 0.490 / 0.564 ms against 0.469 / 0.487 /
+// 0.650 ms of dg::stage_kernel.  Variants that were built and measured slower: the helper
 // also evaluating the N faces of all M columns (one warp's dependent chains became the critical path: 0.53 / 0.57 /
 // 0.65), the helper computing c_s^2 and gravity of the volume nodes with a two-slot tile ring to make room for them
 // (0.47 / 0.50 / 0.64).
@@ -322,13 +324,14 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
     }
     riemann2<FLUX, EOS, 1>(UNq, GNo, lamNo, aU, aG, aLam, HNq);
   };
-  // Balance between the schedulers (M = 5).  Warp slots are handed out in order (two blocks of six: slots 0..5 and
-  // 6..11, scheduler = slot mod 4), so in both blocks workers 0, 2, 4 sit three to a scheduler and workers 1, 3 share
-  // theirs with one other worker and a helper that idles most of the row.  Workers 1 and 3 therefore also do the N
-  // face of columns 0 and M - 1 (first thing in their Y phase, through sHS) and workers 0 and M - 1 skip theirs:
-  // 3 x 0.85 against 2 x 1.15 + helper instead of 3 x 1 against 2 x 1 + helper.  Correct under any slot layout.
+  // Balance between the warps (M = 5).  A block's warps 0..5 sit on schedulers (s, s+1, s+2, s+3, s, s+1) (%warpid mod 4
+  // over the 2048 blocks of a launch; s uniform in 0..3, so how the two blocks of an SM overlap varies): workers 0 and
+  // 4 always share a scheduler.  Workers 1 and 3 therefore also do the N face of columns 0 and M - 1 (first thing in
+  // their Y phase, through sHS) and workers 0 and M - 1 skip theirs.  Found by measurement, with per-warp clock traces
+  // of the row phases: before, workers 0 / 4 / 2 were last at the end-of-row barrier; other assignments (workers 2 and
+  // 3 as takers; worker 1 taking column 2 as well) were slower.  Correct under any slot layout.
   // Measured at 1024^2: first / middle stage 0.450 / 0.490 ms instead of 0.464 / 0.494; in the stages whose helper also
-  // carries the CFL reduction its scheduler has no room to spare (last stage 0.582 instead of 0.566), so not there.
+  // carries the CFL reduction: last stage 0.582 instead of 0.566, so not there.
   constexpr bool REBAL = M == 5 && !do_cfl;
   const bool donor = REBAL && (w == 0 || w == M - 1);
   const bool taker = REBAL && (w == 1 || w == M - 2);
