@@ -52,6 +52,8 @@ CASES.append(dict(nx=5, ny=3, m=3, eos=0, bc=0, gravity=False))             # sm
 CASES.append(dict(nx=32, ny=1, m=2, eos=0, bc=0, gravity=False))            # single row, exact block
 CASES.append(dict(nx=1, ny=1, m=4, eos=0, bc=0, gravity=False))             # one cell, its own neighbour
 CASES.append(dict(nx=64, ny=40, m=5, eos=1, bc=2, gravity=True))            # several row segments
+CASES.append(dict(nx=64, ny=40, m=1, eos=1, bc=2, gravity=True))            # order 1 (its own kernel), several row segments
+CASES.append(dict(nx=40, ny=33, m=1, eos=0, bc=0, gravity=False))           # order 1, periodic wrap across segments
 
 
 def _make(case, rk=3, seed=0):
@@ -595,15 +597,17 @@ def test_literal_baseline_disc_runs_with_the_limiter(DG):
 # ------------------------------------------------------------------------------------------------
 # NEXT-4: strips of a domain decomposed along y, halo rows exchanged before every sub-step
 @pytest.mark.parametrize("name,n_strips", [("vortex", 2), ("vortex", 3), ("disc", 4), ("disc_rk5_lim", 3), ("hllc", 2),
-                                           ("disc_rk4", 2)])
+                                           ("disc_rk4", 2), ("vortex_m1", 3), ("disc_m1", 4)])
 def test_strip_decomposition_reproduces_the_undivided_domain(DG, name, n_strips):
     """All strips on one GPU (`strips.LocalStrips`): the stage kernels read the neighbour strip's boundary rows
     from their halo rows.  Grids and boxes with binary-exact spacings, so the strips' node coordinates are the
     undivided domain's to the last bit and the comparison is bitwise; dt (min over strips) as well."""
     from paper_1805_01443_b200 import strips
-    if name == "vortex":
-        p, U = W.vortex(32, 3, rk=3)
+    if name in ("vortex", "vortex_m1"):
+        p, U = W.vortex(32, 1 if name == "vortex_m1" else 3, rk=3)
         p.update(x1=8.0, y1=8.0)                           # dx = 1/4: exact
+    elif name == "disc_m1":
+        p, U = W.disc(64, 1, planet=True, noise=1e-4, half_width=2.0)
     elif name == "disc":
         p, U = W.disc(64, 4, planet=True, noise=1e-4, half_width=2.0)
     elif name == "disc_rk4":
