@@ -593,7 +593,8 @@ stage_kernel(const __grid_constant__ StageArgs A) {
       enext[q] = (edge_src && more) ? ldg_here(edge_src + (size_t)(j + 1) * row_stride + q * 32) : 0.0;
     if (worker) {
       const int r = w;
-      tile_wait(t);
+      // (no wait for tile t here: this warp has seen its mbarrier phase complete already -- as tile t of the S face in
+      // the prologue, or as the row above in the previous row's Y phase; a second try_wait costs ~100 cycles per row)
       const double yr = yc + g.hdy * T.xi[r];
       const double y2e = fma(yr, yr, A.ph.eps2s);
       double acc[4][M];
