@@ -210,6 +210,34 @@ def test_limiter_floor_is_capped_by_the_cell_average():
     assert abs(th1 - (1.0 - 1e-2) / (0.9 * math.sqrt(3.0))) < 1e-15
 
 
+def test_limiter_pressure_floor_is_capped_by_the_cell_average():
+    """Ideal gas, eps_p = min(lim_eps, pbar) (Zhang & Shu 2010: eps = min(1e-13, rhobar, pbar)).  A cell at rest with
+    the uniform pressure p0 = 1e-3 < lim_eps = 1e-2 and a linear, positive density: every point has p = p0 = pbar, so
+    no point is below the floor min(lim_eps, pbar) = pbar and the cell is left alone (theta_2 = 1, coefficients
+    bitwise).  With eps_p = lim_eps every point counts as inadmissible and the segment to the average never reaches
+    p = lim_eps: theta_2 = 0, the density slope would be wiped out.  Mutation caught: eps_p = lim_eps."""
+    m = 2
+    gamma = 1.4
+    p = W.make_params(nx=1, ny=1, order=m, eos=0, gamma=gamma, limiter=1, lim_eps=1e-2)
+    u = np.zeros((4, m, m))
+    u[0, 0, 0] = 1.0
+    u[0, 0, 1] = 0.3                                                       # rho = 1 + 0.3 sqrt(3) xi > 0.48
+    u[0, 1, 0] = -0.2
+    u[3, 0, 0] = 1e-3 / (gamma - 1.0)                                      # E = p0/(gamma-1), no momentum
+    lim, th1, th2 = oracle.limit_cell(p, u)
+    assert th1 == 1.0 and th2 == 1.0
+    assert np.array_equal(lim, u)
+    # with the average pressure above the floor a point below it is pulled to p = lim_eps exactly (linear E, rho = 1:
+    # p is linear along the segment, t = (pbar - eps)/(pbar - p_point))
+    u = np.zeros((4, m, m))
+    u[0, 0, 0] = 1.0
+    u[3, 0, 0] = 1.0 / (gamma - 1.0)                                       # pbar = 1
+    u[3, 0, 1] = 0.7 / (gamma - 1.0)                                       # p(xi) = 1 + 0.7 sqrt(3) xi: p(-1) = -0.212
+    lim, th1, th2 = oracle.limit_cell(p, u)
+    assert th1 == 1.0
+    assert abs(th2 - (1.0 - 1e-2) / (0.7 * math.sqrt(3.0))) < 1e-14
+
+
 # ------------------------------------------------------------------------------------------------
 # C8b + C12: the limiter inside the Butcher-form sub-steps.  Mutation caught: deleting post() in butcher_step.
 def _limiter_points_min_rho(m, cell):
@@ -412,3 +440,15 @@ def test_normalised_torque_hand_value():
     sigma_p = 0.7
     gamma0 = sigma_p * 1.0 * 1.0 * 1e-3 / 0.05 ** 2
     assert abs(r.torque_normalised(0.0, sigma_p) - 1.4 * gam / gamma0) < 1e-12 * abs(gam / gamma0)
+    # every factor of Gamma_0 with a value other than 1: r_p = 1.5 (fourth power), Omega = 0.6 (squared), planet at
+    # phase 0.3
+    rp, om, ph = 1.5, 0.6, 0.3
+    p2 = dict(p, r_planet=rp, omega_planet=om, phase0=ph)
+    r2 = oracle.RefDG(p2)
+    r2.set_state(U)
+    xp, yp = rp * math.cos(ph), rp * math.sin(ph)
+    ddx, ddy = xcell - xp, ycell - yp
+    d3 = (ddx ** 2 + ddy ** 2 + 0.01) ** 1.5
+    gam2 = 3.0 * dx * dx * (xp * ddy - yp * ddx) / d3
+    gamma02 = sigma_p * om ** 2 * rp ** 4 * 1e-3 / 0.05 ** 2
+    assert abs(r2.torque_normalised(0.0, sigma_p) - 1.4 * gam2 / gamma02) < 1e-12 * abs(gam2 / gamma02)

@@ -979,3 +979,47 @@ def test_order5_stage_kernels_agree(DG, over):
     for k in (1, 2):
         assert rel_err(outs[k], outs[0]) < 1e-13
         assert max(abs(a / b - 1.0) for a, b in zip(dts[k], dts[0])) < 1e-13
+
+
+@pytest.mark.parametrize("m", [2, 3, 5])
+def test_limiter_floor_guards_parity(DG, m):
+    """The two guards of the limiter's floor, eps_rho = min(lim_eps, rhobar) and eps_p = min(lim_eps, pbar) (Zhang & Shu
+    2010), on cells built for them (pinned for the oracle in tests/test_oracle_pins_r2.py): a cell whose average
+    density lies below lim_eps with a negative point (theta_1 = 0); a cell at rest whose average pressure lies below
+    lim_eps, with a pressure slope (eps_p = pbar: the segment to the average meets p = pbar at t = 0, theta_2 = 0);
+    a cell with a negative-pressure point and the average above the floor.
+    (The oracle's pin for eps_p uses a cell of exactly uniform pressure, which must stay untouched; that is a tie
+    p(x) = eps_p decided by the last bit of the cell average -- exact for the oracle's mode (0,0), a quadrature sum
+    in the nodal kernel -- and therefore no parity case.)"""
+    gamma = 1.4
+    nx, ny = 40, 3
+    p = W.make_params(nx=nx, ny=ny, order=m, eos=0, gamma=gamma, bc=0, rk=3, limiter=1, lim_eps=1e-2)
+    U = np.zeros((ny, nx, 4, m, m))
+    U[..., 0, 0, 0] = 1.0
+    U[..., 3, 0, 0] = 1.0 / (gamma - 1.0)
+    for i in range(nx):
+        kind = i % 4
+        if kind == 1:                                    # rhobar < lim_eps, rho negative at xi = -1
+            U[:, i, 0, 0, 0] = 1e-3
+            U[:, i, 0, 0, 1] = 2e-3
+            U[:, i, 3, 0, 0] = 1e-3 / (gamma - 1.0)
+        elif kind == 2:                                  # pbar = 1e-3 < lim_eps, pressure and density slopes
+            U[:, i, 0, 0, 1] = 0.3
+            U[:, i, 0, 1, 0] = -0.2
+            U[:, i, 3, 0, 0] = 1e-3 / (gamma - 1.0)
+            U[:, i, 3, 0, 1] = 2e-4 / (gamma - 1.0)
+        elif kind == 3:                                  # pbar = 1, p(-1) < 0
+            U[:, i, 3, 0, 1] = 0.7 / (gamma - 1.0)
+    ref = oracle.RefDG(p, omp=True)
+    ref.set_state(U)
+    ref.limit()
+    out_ref = ref.get_state()
+    g = DG(p)
+    g.set_state(dev(U))
+    g.limit()
+    out = g.get_state().cpu().numpy()
+    assert np.abs(out - out_ref).max() < 1e-12
+    for kind in (1, 2):                                  # collapsed to the cell average: theta = 0
+        hi = out_ref[:, kind::4].reshape(ny, -1, 4, m * m)[..., 1:]
+        assert np.abs(hi[:, :, 0]).max() == 0.0
+    assert np.abs(out_ref[:, 3::4, 3].reshape(ny, -1, m * m)[..., 1:]).max() > 0.1      # scaled, not collapsed
