@@ -452,3 +452,27 @@ def test_normalised_torque_hand_value():
     gam2 = 3.0 * dx * dx * (xp * ddy - yp * ddx) / d3
     gamma02 = sigma_p * om ** 2 * rp ** 4 * 1e-3 / 0.05 ** 2
     assert abs(r2.torque_normalised(0.0, sigma_p) - 1.4 * gam2 / gamma02) < 1e-12 * abs(gam2 / gamma02)
+
+
+# ------------------------------------------------------------------------------------------------
+# Step (v) of the paper's loop: the time advances by the step just taken, and the planet of the
+# next step's source term sits where that time puts it.  Mutation caught: `c->t += dt` dropped from the step.
+def test_time_advances_and_the_planet_moves_with_it():
+    p, U = W.disc(12, 2, planet=True, noise=0.0)
+    p = dict(p, q_planet=1e-2, t0=0.25)
+    a = oracle.RefDG(p)
+    a.set_state(U)
+    assert a.time == 0.25
+    dt = a.cfl_dt(0.2)
+    a.step(dt)
+    assert a.time == 0.25 + dt
+    a.step(dt)
+    assert a.time == 0.25 + dt + dt
+    # the same two steps with the clock put back by hand after the first one: the second step then evaluates the
+    # planet's gravity dt too early, and the result differs
+    b = oracle.RefDG(p)
+    b.set_state(U)
+    b.step(dt)
+    b.time = 0.25
+    b.step(dt)
+    assert np.abs(b.get_state() - a.get_state()).max() > 1e-12
