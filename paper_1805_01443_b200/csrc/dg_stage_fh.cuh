@@ -11,11 +11,12 @@
 //         flux -> sHX, one row ahead.  dg::stage_kernel does this on lanes 0 and 31 of every worker behind divergent
 //         branches (~130 of its ~1400 instructions per row) and carries the prefetched lines in 20 registers;
 //       * the S face of the segment's first row (prologue);
-//       * TMA issue, mbarrier waits for the tiles, L2 prefetches, the fused CFL reduction.
+//       * TMA issue, mbarrier waits for the tiles, L2 prefetches, the fused CFL reduction, the cells' wave-killing
+//         factors (last stage).
 //
 // Why a sixth warp is free: five warps of 168 registers make two blocks per SM = 10 warps; 12 x 168 x 32 registers still
 // fit the register file (3 warps per scheduler), and the shared memory of a block does not grow (114.6 KB).
-// Measured at 1024^2, order 5 (B200): first / middle / last stage 0.450 / 0.490 / 0.564 ms against 0.469 / 0.487 /
+// Measured at 1024^2, order 5 (B200): first / middle / last stage 0.450 / 0.490 / 0.554 ms against 0.469 / 0.487 /
 // 0.650 ms of dg::stage_kernel.  Variants that were built and measured slower: the helper
 // also evaluating the N faces of all M columns (one warp's dependent chains became the critical path: 0.53 / 0.57 /
 // 0.65), the helper computing c_s^2 and gravity of the volume nodes with a two-slot tile ring to make room for them
@@ -444,11 +445,9 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
 #pragma unroll
           for (int r = 0; r < M; ++r) acc[v][r] = 0.0;
         // wave-killing factors of this cell (row a12): out <- f0 u0 + ft out
-        double f0 = 0.0, ft = 1.0;
+        double f0 = 0.0, ft = 1.0;                 // (from the helper, once the N face is done)
         bool damp = false;
-        if (do_damp && (KIND != K_GENL || A.D.on))
-          damp = damp_factors(A.D, sqrt_fast(fma(xc, xc, yc * yc) + 1e-300), f0, ft);   // + tiny: a centre at the origin
-        constexpr bool early_q0 = do_damp;
+        constexpr bool early_q0 = false;
         double z0[4][M];
         if (early_q0) {
           const double* __restrict__ q0e = A.q0 + j * row_stride + (size_t)ib * BS + lane;
@@ -512,6 +511,11 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
         } else {
           if (!taker) bar_sync_named(3 + w, 64);
           n_face(t, j, q, UN, HN);
+        }
+        if (do_damp) {                           // the cell's wave-killing factors: one evaluation per row, by the helper
+          f0 = sHS[lane];
+          ft = sHS[32 + lane];
+          damp = f0 != 0.0;
         }
 
         // modal update in nodal form + RK combination (rows a8, a9) and store
@@ -591,6 +595,19 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
           if (!(sp >= 0.0)) sp = __longlong_as_double(0x7ff0000000000000LL);   // NaN -> +inf
         }
         spmax = fmax(spmax, sp);                 // per lane; reduced once after the last row
+      }
+      // wave-killing factors of the row's cells (row a12): out <- f0 u0 + ft out.  One evaluation per cell
+      // here instead of one per column warp; the workers read them after they have synchronised on barrier 3 + w
+      // (sHS is free in these stages: the N-face hand-over runs only in stages without the CFL reduction)
+      if (do_damp) {
+        double f0 = 0.0, ft = 1.0;
+        const double ycj = g.y0 + (j + 0.5) * g.dy;
+        if (KIND != K_GENL || A.D.on) {
+          if (!damp_factors(A.D, sqrt_fast(fma(xc, xc, ycj * ycj) + 1e-300), f0, ft)) { f0 = 0.0; ft = 1.0; }   // + tiny: a centre at the origin
+        }
+        sHS[lane] = f0;
+        sHS[32 + lane] = ft;
+        __threadfence_block();
       }
       tile_wait(t + 1);                          // sent a whole row ago; the workers' N faces and the next row read it
 #pragma unroll
