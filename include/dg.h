@@ -209,6 +209,32 @@ int dg_probe_fp64_peak(dg_ctx*, double* tflops /*HOST*/);
 const char* dg_last_error(const dg_ctx*);
 void dg_destroy(dg_ctx*);
 
+/* --- An entry point that allocates nothing, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it): no context, no workspace, no host allocation either. ---
+ *
+ * dg_torque_static: the torque of Eq.(6), exactly as dg_torque defines it (M_n = cell-average
+ * density x cell area, r_n = cell centre, planet at r_p (cos, sin)(omega_p t + phase0), softening eps_p), computed
+ * straight from a modal state in the external layout (mode (0,0) = the cell average).
+ *   params : HOST.  Read: nx, ny, x0, x1, y0, y1, order, gm_star, r_planet, eps_planet, omega_planet, phase0.
+ *   U      : DEVICE, [ny][nx][4][m][m] doubles (m = order), the caller's; not changed.
+ *   out    : DEVICE, 3 doubles, the caller's: out[0] = Gamma_z, out[1] = a_x, out[2] = a_y (Gamma_z = x_p a_y - y_p a_x).
+ *   cuda_stream : cudaStream_t; two kernels are enqueued on it, nothing is synchronised, nothing is copied to the host.
+ * The scratch of the reduction (per-block partial sums) is a file-scope __device__ array inside the library:
+ * 2 x DG_STATIC_MAX_BLOCKS doubles = 1 MiB, held by every GPU that loads the library until the process exits.  A
+ * thread block covers 32 x 32 cells, so grids with ceil(nx/32) x ceil(ny/32) <= DG_STATIC_MAX_BLOCKS are accepted (up to
+ * 8192 x 8192 cells); larger ones return DG_ENOSPC (use dg_torque: its scratch is in the workspace).  Every call on a
+ * device shares that array; it is never cleared and need not be (a call overwrites every slot it later reads), but
+ * calls that overlap on the GPU -- different streams with no ordering between them -- race on it: order them.
+ * The array's device address is looked up (cudaGetSymbolAddress) once per device, with that device current: on the first
+ * dg_torque_static call there, or by dg_static_setup() -- call that before a stream capture begins.
+ * Errors: DG_EINVAL (null / misaligned pointer, bad sizes), DG_ENOSPC, DG_ECUDA; message in dg_static_last_error()
+ * (per host thread). */
+#define DG_STATIC_MAX_BLOCKS 65536
+int dg_static_setup(void);
+int dg_torque_static(const dg_params* params /*HOST*/, const double* U /*DEVICE*/, double t,
+                     double* out /*DEVICE, 3 doubles*/, void* cuda_stream);
+const char* dg_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

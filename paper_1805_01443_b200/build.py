@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdg.so")
-SOURCES = ["dg_api.cu"] + [f"dg_stage_m{m}{f}.cu" for m in (5, 4, 3, 2, 1) for f in ("", "f")]
+SOURCES = ["dg_api.cu", "dg_static.cu"] + [f"dg_stage_m{m}{f}.cu" for m in (5, 4, 3, 2, 1) for f in ("", "f")]
 DEPS = SOURCES + ["dg_kernels.cuh", "dg_stage_fh.cuh", "dg_stage_m1fv.cuh", "dg_stage_launch.cuh", "dg_tables.h", "dg_limit.cuh",
                   os.path.join("..", "..", "include", "dg.h")]
 OBJ_DIR = os.path.join(HERE, "build")

@@ -20,6 +20,7 @@ EXPORTS = [
     "dg_stage_time_ms", "dg_stage_times_ms", "dg_probe_fp64_peak", "dg_last_error", "dg_destroy",
     "dg_rk_stages", "dg_limit", "dg_torque", "dg_torque_normalised",
     "dg_step_begin", "dg_substep", "dg_substep_part", "dg_step_end", "dg_halo_layout",
+    "dg_static_setup", "dg_torque_static", "dg_static_last_error",
 ]
 
 
@@ -90,12 +91,40 @@ def load_library(path: str | None = None):
         "dg_halo_layout": (i, [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
         "dg_rk_stages": (i, [i]), "dg_limit": (i, [vp]), "dg_torque": (i, [vp, d, C.POINTER(d)]),
         "dg_torque_normalised": (i, [vp, d, d, C.POINTER(d)]),
+        "dg_static_setup": (i, []), "dg_torque_static": (i, [PP, vp, d, vp, vp]),
+        "dg_static_last_error": (C.c_char_p, []),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
         fn.restype, fn.argtypes = res, args
     _lib = L
     return L
+
+
+def static_setup():
+    """dg_static_setup: look up the library's static scratch on the current device (once per device)."""
+    L = load_library()
+    if L.dg_static_setup() != 0:
+        raise DGError(L.dg_static_last_error().decode())
+
+
+def torque_static(params: dict, U, t: float, out, stream=None):
+    """dg_torque_static: torque of Eq.(6) from a modal DEVICE state ``U`` into the DEVICE tensor ``out`` (3 doubles),
+    on ``stream`` (default: torch's current stream).  No context, no workspace, nothing allocated, nothing synchronised."""
+    import torch
+    L = load_library()
+    for x in (U, out):
+        if not (x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()):
+            raise DGError("torque_static: U and out must be contiguous fp64 CUDA tensors")
+    m = int(params["order"])
+    if U.numel() != int(params["ny"]) * int(params["nx"]) * 4 * m * m or out.numel() < 3:
+        raise DGError("torque_static: U must hold ny*nx*4*m*m doubles and out at least 3")
+    ps = params_struct(params)
+    s = stream if stream is not None else torch.cuda.current_stream()
+    e = L.dg_torque_static(C.byref(ps), U.data_ptr(), float(t), out.data_ptr(), s.cuda_stream)
+    if e != 0:
+        raise DGError(f"dg_torque_static: {e}: {L.dg_static_last_error().decode()}")
+    return out
 
 
 class DG:
