@@ -21,6 +21,11 @@ NVCC_COMPILE = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "--extended-lambda", "-Xcompiler", "-fPIC", "-c",
 ]
+# Order 1 (dg_stage_m1fv.cuh) repeats its row body six times so that its row buffers rotate by renaming; left to itself
+# the compiler contracts a * b + c into an FMA in some copies and not in others, and the result of a row would depend
+# on its position in the segment (strips of a decomposed domain would no longer reproduce the undivided domain bitwise).
+# Without contraction only the FMAs the source spells out are FMAs, in every copy.
+PER_SOURCE = {"dg_stage_m1.cu": ["-fmad=false"], "dg_stage_m1f.cu": ["-fmad=false"]}
 NVCC_LINK = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static"]
 
 
@@ -40,7 +45,7 @@ def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
     procs = []
     for src in SOURCES:
         obj = os.path.join(OBJ_DIR, src.replace(".cu", ".o"))
-        cmd = [nvcc, *NVCC_COMPILE, *extra_flags, *(["-Xptxas", "-v"] if verbose else []),
+        cmd = [nvcc, *NVCC_COMPILE, *PER_SOURCE.get(src, []), *extra_flags, *(["-Xptxas", "-v"] if verbose else []),
                os.path.join(CSRC, src), "-o", obj]
         procs.append((src, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     objs = []

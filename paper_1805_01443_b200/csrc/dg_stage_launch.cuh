@@ -48,8 +48,8 @@ cudaError_t launch_stage_variant_fh(const StageArgs& A, dim3 grid, cudaStream_t 
 template <int M, int EOS, int GRAV, int KIND, int FLUX>
 cudaError_t launch_stage_variant(const StageArgs& A, dim3 grid, cudaStream_t stream) {
   if constexpr (M == 1) {                        // order 1: the register-only kernel (dg_stage_m1fv.cuh), one warp per segment of rows
-    if (A.impl != 1 && A.g.nx % 32 != 1) {
-      stage_kernel_m1<EOS, GRAV, KIND, FLUX><<<dim3(grid.x, (grid.y + M1_WARPS - 1) / M1_WARPS), M1_WARPS * 32, 0, stream>>>(A);
+    if (A.impl != 1) {
+      stage_kernel_m1<EOS, GRAV, KIND, FLUX><<<dim3((A.g.nx + M1_OWN - 1) / M1_OWN, (grid.y + M1_WARPS - 1) / M1_WARPS), M1_WARPS * 32, 0, stream>>>(A);
       return cudaGetLastError();
     }
   }
