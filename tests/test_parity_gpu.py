@@ -54,6 +54,13 @@ CASES.append(dict(nx=1, ny=1, m=4, eos=0, bc=0, gravity=False))             # on
 CASES.append(dict(nx=64, ny=40, m=5, eos=1, bc=2, gravity=True))            # several row segments
 CASES.append(dict(nx=64, ny=40, m=1, eos=1, bc=2, gravity=True))            # order 1 (its own kernel), several row segments
 CASES.append(dict(nx=40, ny=33, m=1, eos=0, bc=0, gravity=False))           # order 1, periodic wrap across segments
+# order 1 owns 30 cells per warp (lanes 1..30; lanes 0 and 31 hold the x-neighbours): exactly one warp, one owned cell in
+# the last warp, a warp boundary inside the domain, a cell that is both of its own neighbours, frozen traces on both sides
+CASES.append(dict(nx=30, ny=5, m=1, eos=0, bc=0, gravity=False))
+CASES.append(dict(nx=31, ny=6, m=1, eos=1, bc=2, gravity=True))
+CASES.append(dict(nx=61, ny=7, m=1, eos=0, bc=1, gravity=True))
+CASES.append(dict(nx=1, ny=3, m=1, eos=0, bc=0, gravity=False))
+CASES.append(dict(nx=2, ny=2, m=1, eos=1, bc=2, gravity=True))
 
 
 def _make(case, rk=3, seed=0):
@@ -521,7 +528,9 @@ def test_full_size_next_rows(DG):
 # ------------------------------------------------------------------------------------------------
 # NEXT-4: HLLC (ideal gas) / HLL (isothermal) flux option
 @pytest.mark.parametrize("rk", [3, 5])
-@pytest.mark.parametrize("case", NEXT_CASES + [dict(nx=1, ny=1, m=4, eos=0, bc=0, gravity=False)], ids=_id)
+@pytest.mark.parametrize("case", NEXT_CASES + [dict(nx=1, ny=1, m=4, eos=0, bc=0, gravity=False),
+                                              dict(nx=61, ny=7, m=1, eos=0, bc=1, gravity=True),
+                                              dict(nx=31, ny=6, m=1, eos=1, bc=2, gravity=True)], ids=_id)
 def test_hllc_parity(DG, case, rk):
     p, U = _make(case, rk=rk, seed=13)
     p["flux"] = 1
@@ -548,6 +557,22 @@ def test_hllc_parity(DG, case, rk):
     g3.set_state(dev(U))
     if case["m"] > 1 and case["nx"] > 1:
         assert np.abs(g3.rhs(0.21).cpu().numpy() - L).max() > 1e-6
+
+
+@pytest.mark.parametrize("flux", [0, 1])
+def test_order1_conserves_across_warp_and_segment_boundaries(DG, flux):
+    """Order 1 (dg_stage_m1fv.cuh): the x-face between two warps' cells is evaluated by both warps, the y-face between two
+    row segments by one; on a periodic box without sources the totals move only by the rounding of the update."""
+    p, U = W.random_smooth(95, 23, 1, seed=19, bc=0, rk=3)
+    p["flux"] = flux
+    g = DG(p)
+    g.set_tuning(1, 4)
+    g.set_state(dev(U))
+    tot0 = U[..., 0, 0].sum(axis=(0, 1))
+    for _ in range(10):
+        g.step(g.cfl_dt(0.2))
+    tot1 = g.get_state().cpu().numpy()[..., 0, 0].sum(axis=(0, 1))
+    assert (np.abs(tot1 - tot0) / np.abs(U[..., 0, 0]).sum(axis=(0, 1))).max() < 5e-15
 
 
 def test_hllc_100_steps_and_conservation(DG):
