@@ -12,12 +12,13 @@
 
 namespace dg {
 
-// Thread blocks per SM the register allocation aims at; shared memory (4 tiles + tables per block)
+// Thread blocks per SM the register allocation aims at (order 3: 4 blocks of 160 registers beat 5 of 128, which spill);
+// shared memory (4 tiles + tables per block)
 // allows exactly this many on a 227 KB SM for M = 5, 4 and is not the limit below.
 template <int M> struct StageMinBlocks;
 template <> struct StageMinBlocks<1> { static constexpr int value = 16; };
 template <> struct StageMinBlocks<2> { static constexpr int value = 8; };
-template <> struct StageMinBlocks<3> { static constexpr int value = 5; };
+template <> struct StageMinBlocks<3> { static constexpr int value = 4; };
 template <> struct StageMinBlocks<4> { static constexpr int value = 3; };
 template <> struct StageMinBlocks<5> { static constexpr int value = 2; };
 
