@@ -79,6 +79,32 @@ def test_workspace_sizing_and_validation(lib):
     lib.dg_destroy(None)
 
 
+def test_static_entry_point_validates_before_touching_the_device(lib):
+    """dg_torque_static (the entry point that allocates nothing): null / misaligned pointers, bad sizes and grids beyond
+    the static scratch are rejected on the host, with a message, before any CUDA call."""
+    from paper_1805_01443_b200 import workloads as W
+    from paper_1805_01443_b200.dg import params_struct
+    p, _ = W.vortex(32, 2)
+    ps = params_struct(p)
+    assert lib.dg_torque_static(None, 64, 0.0, 64, None) == -1
+    assert lib.dg_torque_static(C.byref(ps), None, 0.0, 64, None) == -1
+    assert lib.dg_torque_static(C.byref(ps), 64, 0.0, None, None) == -1
+    assert b"null" in lib.dg_static_last_error()
+    assert lib.dg_torque_static(C.byref(ps), 68, 0.0, 64, None) == -1          # U not 8-byte aligned
+    assert b"aligned" in lib.dg_static_last_error()
+    for bad in (dict(order=0), dict(order=6), dict(nx=0), dict(ny=-1), dict(x1=p["x0"])):
+        assert lib.dg_torque_static(C.byref(params_struct(dict(p, **bad))), 64, 0.0, 64, None) == -1, bad
+    assert lib.dg_torque_static(C.byref(ps), 64, float("nan"), 64, None) == -1
+    # 65 536 blocks of 32 x 32 cells is the limit: 8192 x 8192 cells pass the size check (and then fail on the missing
+    # device here, or on the bad pointer never being touched), one more block does not
+    big = params_struct(dict(p, nx=8192 + 1, ny=8192))
+    assert lib.dg_torque_static(C.byref(big), 64, 0.0, 64, None) == -2         # DG_ENOSPC
+    msg = lib.dg_static_last_error().decode()
+    assert "DG_STATIC_MAX_BLOCKS" in msg and "65792" in msg
+    hdr = open(HEADER).read()
+    assert re.search(r"#define\s+DG_STATIC_MAX_BLOCKS\s+65536\b", hdr)
+
+
 def test_no_cpu_fallback():
     """Without a device the product refuses to run (it must not route through the oracle)."""
     import torch
