@@ -180,7 +180,8 @@ long long dg_launch_count(const dg_ctx*);
 
 /* Tuning knobs (all have defaults; DG_EINVAL on unknown key or bad value).
  *   DG_TUNE_ROWS_PER_CTA : rows of cells one thread block marches over in the stage kernel (default: 4..16,
- *                          chosen at dg_init so that the grid gives about four waves of blocks)
+ *                          chosen at dg_init: long segments re-read fewer neighbour rows, and the number of blocks
+ *                          should come close to a multiple of what the GPU holds at once)
  *   DG_TUNE_FUSED_CFL    : 1 = the last RK stage also reduces the CFL wave speed (default), 0 = separate kernel */
 #define DG_TUNE_ROWS_PER_CTA 1
 #define DG_TUNE_FUSED_CFL    2

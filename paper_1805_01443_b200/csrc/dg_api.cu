@@ -618,16 +618,29 @@ int dg_init(const dg_params* p, void* workspace, size_t ws_bytes, void* cuda_str
   c->has_state = false;
   c->wmax_valid = false;
   c->t = p->t0;
-  // rows of cells per thread block: enough blocks for ~4 waves over the SMs, between 4 and 16 rows
-  // (16 rows re-read 2/16 of u^(s-1) as halo; small grids fit L2 and want more, shorter blocks:
-  // 256^2 order 3 runs 0.021 ms per stage at 4 rows, 0.042 at 16)
+  // Rows of cells a thread block (order 1: a warp) marches over, between 4 and 16.  Two things pull against each other:
+  // a segment of r rows also reads the row below and the row above it and pays its prologue once, ~ (r + 1)/r of the
+  // work, and the last wave of thread blocks leaves SMs idle unless the block count is close to a multiple of what the
+  // GPU holds at once (1024^2, order 1: 13 rows make 700 blocks for 592 slots, two waves at 59 %; 16 rows make 560, one
+  // wave: 0.036 against 0.029 ms per stage).  Take the r with the best product of the two.  Small grids come out with
+  // short segments (256^2 order 3: 4 rows, 0.021 ms per stage; 16 rows, 0.042), large ones with 16.
   {
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    static const int blocks_per_sm[MAXM + 1] = {0, 16, 8, 5, 3, 2};
-    const long tiles = (long)L.nbx * p->ny;
-    long rows = tiles / (4L * sms * blocks_per_sm[p->order]);
-    c->rows_per_cta = (int)std::max(4L, std::min(16L, rows));
+    // thread blocks of the default stage kernel an SM holds (dg_stage_launch.cuh; order 1: blocks of 4 warps)
+    static const int blocks_per_sm[MAXM + 1] = {0, 4, 8, 4, 3, 2};
+    const long cols = p->order == 1 ? (p->nx + 29) / 30 : L.nbx;
+    const long slots = (long)sms * blocks_per_sm[p->order];
+    double best = -1.0;
+    int best_r = 4;
+    for (int r = 4; r <= 16; ++r) {
+      const long segs = (p->ny + r - 1) / r;
+      const long blocks = cols * (p->order == 1 ? (segs + 3) / 4 : segs);
+      const long waves = (blocks + slots - 1) / slots;
+      const double score = (double)blocks / (double)(waves * slots) * r / (r + 1.0);
+      if (score >= best) { best = score; best_r = r; }
+    }
+    c->rows_per_cta = best_r;
   }
   c->fused_cfl = 1;
   c->rk4_low_storage = 1;
