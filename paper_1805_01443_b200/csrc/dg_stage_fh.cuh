@@ -10,7 +10,6 @@
 //         from L2 (requested two rows ahead), the own edge cell's line from the tile, boundary conditions, Riemann
 //         flux -> sHX, one row ahead.  dg::stage_kernel does this on lanes 0 and 31 of every worker behind divergent
 //         branches (~130 of its ~1400 instructions per row) and carries the prefetched lines in 20 registers;
-//       * the S face of the segment's first row (prologue);
 //       * TMA issue, mbarrier waits for the tiles, L2 prefetches, the fused CFL reduction, the cells' wave-killing
 //         factors (last stage).
 //
@@ -114,8 +113,8 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
   double* tiles = smem;
   double* sN = tiles + NS * BS;                  // u^n landing buffer -> a u^n + x-part of beta N -> (fused CFL) partial averages
   double* sRi = sN + BS;                         // [r][q][lane]: 1/sqrt(x^2+y^2+eps^2) at the row's volume nodes
-  double* sHS = sRi + M * M * 32;                // [v][q][lane]: S-face fluxes (x2) of the segment's first row (prologue); then
-                                                 // the N-face fluxes one worker evaluates for another (M = 5)
+  double* sHS = sRi + M * M * 32;                // [v][q][lane]: the N-face fluxes one worker evaluates for another (M = 5);
+                                                 // the wave-killing factors of the row's cells (last stage)
   double* sHX = sHS + 4 * M * 32;                // [row parity][r][side][v]: W flux of cell 0, E flux of the last cell
   uint64_t* mbar = reinterpret_cast<uint64_t*>(sHX + 2 * M * 8);   // [NS] tiles, u^n
 
@@ -273,28 +272,23 @@ stage_kernel_fh(const __grid_constant__ StageArgs A) {
     nb_load(j0);
     tile_wait(0);
     tile_wait(1);
-    {                                            // S face of the first row, all M columns
-      const double* lo = tile_row(0) != -1 ? tiles + lane : nullptr;
-      const double* hi = tiles + BS + lane;
-      const double* btr = A.btrS + (size_t)(ib * 4) * M * 32 + lane;
-#pragma unroll 1
-      for (int q = 0; q < M; ++q) {
-        double H[4];
-        y_face<M, EOS, FLUX>(A, lo, hi, btr, q, xc + g.hdx * T.xi[q], g.y0 + j0 * g.dy, H);
-#pragma unroll
-        for (int v = 0; v < 4; ++v) sHS[(v * M + q) * 32 + lane] = H[v];
-      }
-    }
     edge_faces(j0, tiles + BS, sHX);
     if (j0 + 1 < j1) nb_load(j0 + 1);            // consumed in the first row's iteration
   }
-  __syncthreads();
+  // S face of the segment's first row: every worker its own column, straight into its registers, while the helper
+  // does the tile-edge faces.  (The helper used to evaluate all M columns one after the other with the workers waiting
+  // at the barrier below: 6 % of all warp stall samples of the first stage sat on that barrier, about one row's time
+  // per 16-row segment.)  The workers wait for the two tiles on the tiles' own mbarriers -- here and nowhere else.
   double HS[4] = {0, 0, 0, 0};                   // numerical flux (x2) through the row's S face, column q = w
   if (worker) {
-#pragma unroll
-    for (int v = 0; v < 4; ++v) HS[v] = sHS[(v * M + w) * 32 + lane];
+    tile_wait(0);
+    tile_wait(1);
+    const double* lo = tile_row(0) != -1 ? tiles + lane : nullptr;
+    const double* hi = tiles + BS + lane;
+    const double* btr = A.btrS + (size_t)(ib * 4) * M * 32 + lane;
+    y_face<M, EOS, FLUX>(A, lo, hi, btr, w, xc + g.hdx * T.xi[w], g.y0 + j0 * g.dy, HS);
   }
-  __syncthreads();                               // tile 0's slot may be overwritten
+  __syncthreads();                               // sHX of the first row is written; tile 0's slot may be overwritten
 
   // N face of column qn of the row whose tile is tlo: the row's trace UNq at eta = +1 against the S trace of the row
   // above (tile tlo + 1) or the boundary condition
