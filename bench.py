@@ -477,7 +477,7 @@ def run_cuda_arm(args) -> dict | None:
         "clocks": clocks,
         "roofline": {
             "bound": "hbm", "kernel": ("dg::stage_kernel_fh<M=%d> (fused RK stage, M worker warps + a helper warp: rows a1-a9, a11, a12 + a10 in the last)"
-                                       if (m in (3, 5) and STAGE_IMPL != 1) else
+                                       if (m >= 3 and STAGE_IMPL != 1) else
                                        "dg::stage_kernel<M=%d> (fused RK stage: rows a1-a9, a11, a12 + a10 in the last)") % m,
             "stage_impl": STAGE_IMPL,
             "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

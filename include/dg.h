@@ -188,11 +188,11 @@ long long dg_launch_count(const dg_ctx*);
 #define DG_TUNE_GEN_PREFETCH 3   /* general sub-steps: L2 prefetch of the earlier stage states: 0 none, 1 at the start of the row, 2 a row ahead, 3 between the x and y phases of the row (default) */
 #define DG_TUNE_RK4_FORM     4   /* rk 4, limiter off: 1 = Table 1's scheme in its low-storage (Shu-Osher) form, from the
                                    printed tableau's row ratios (default); 0 = the generic state form */
-#define DG_TUNE_STAGE_IMPL   5   /* which fused stage kernel runs: 0 = the default (orders 3 and 5: the kernel with the helper
+#define DG_TUNE_STAGE_IMPL   5   /* which fused stage kernel runs: 0 = the default (orders 3 to 5: the kernel with the helper
                                    warp, dg_stage_fh.cuh, except for the sub-steps of the general schemes that gather earlier
-                                   stage states; order 1: the register-only kernel, dg_stage_m1fv.cuh; orders 2 and 4: M
+                                   stage states; order 1: the register-only kernel, dg_stage_m1fv.cuh; order 2: M
                                    worker warps), 1 = M worker warps (dg::stage_kernel) at every order, 2 = like 0 but
-                                   the helper-warp kernel for every sub-step of orders 3 and 5.  Same results to a few ulp. */
+                                   the helper-warp kernel for every sub-step of orders 3 to 5.  Same results to a few ulp. */
 int dg_set_tuning(dg_ctx*, int key, int value);
 
 /* Average-duration probe: enqueue CUDA events around the stage kernels of the next dg_step calls.

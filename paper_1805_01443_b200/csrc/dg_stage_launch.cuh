@@ -24,10 +24,10 @@ template <> struct StageMinBlocks<5> { static constexpr int value = 2; };
 
 // Orders whose default stage kernel is the one with the face-helper warp (dg_stage_fh.cuh).  Order 5: M worker warps
 // of 168 registers leave the schedulers unevenly filled.  Order 3: 4 blocks of 3 + 1 warps at 128 registers, 4 % faster
-// than 4 blocks of 3 warps at 160 (A/B on one box, 1024^2 and 2048^2).  Order 4 would need 136 registers for 3 blocks of
-// 5 warps and spills (-1 % / +2 %), order 2 with a third warp (6 blocks, 96 registers) is 17-25 % slower: they keep
-// dg::stage_kernel.
-template <int M> struct StageFaceHelper { static constexpr bool value = M == 5 || M == 3; };
+// than 4 blocks of 3 warps at 160, and another 4 % since the workers evaluate the segment's first S face themselves.
+// Order 4: 3 blocks of 4 + 1 warps at 136 registers (24-40 B of spills), +2 % at 1024^2 and +0.4 % at 2048^2 (A/B in
+// one process).  Order 2 with a third warp (6 blocks, 96 registers) is 17-25 % slower and keeps dg::stage_kernel.
+template <int M> struct StageFaceHelper { static constexpr bool value = M >= 3; };
 
 constexpr int kMaxDevices = 64;
 

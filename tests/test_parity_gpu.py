@@ -977,11 +977,11 @@ def test_dist_strip_two_gpus_bitwise(DG):
         assert t == g.time
 
 
-@pytest.mark.parametrize("m", [5, 3])
+@pytest.mark.parametrize("m", [5, 4, 3])
 @pytest.mark.parametrize("over", [{}, {"rk": 2}, {"rk": 4}, {"rk": 5}, {"rk": 5, "limiter": 1}, {"flux": 1},
                                   {"eos": 0, "bc": 0}, {"bc": 1}], ids=str)
 def test_order5_stage_kernels_agree(DG, over, m):
-    """Orders 5 and 3 have two fused stage kernels (DG_TUNE_STAGE_IMPL, include/dg.h): dg::stage_kernel (M worker warps)
+    """Orders 3, 4 and 5 have two fused stage kernels (DG_TUNE_STAGE_IMPL, include/dg.h): dg::stage_kernel (M worker warps)
     and dg::stage_kernel_fh (M workers + a helper warp; the default except for the K_GEN sub-steps).  Same arithmetic:
     after six steps with dt recomputed they agree to a few ulp, on a ragged grid (70 = 2 tiles + 6 cells wide) with
     every boundary type, both closures, every RK scheme and the limiter; and each matches the oracle at 1e-12 per
